@@ -1,0 +1,199 @@
+// Capsule copy kernel: one launch moves every (row, segment) of a named buffer set.
+//
+// PAPER.md:117-132 (Algorithm 1) makes snapshot / restore / fork / rollback "a single copy of
+// that buffer set" — Θ(bytes), bandwidth-bound (Table 3).  The paper
+// does not say how its device-to-device copy is issued; here it is ONE kernel driven by a
+// descriptor table (kernel parameter space, or a device-resident table inside captured
+// graphs), so a 24-30 buffer capsule pays one launch, not 30 memcpy nodes.
+//
+// Roofline: HBM.  Algorithmic bytes = 2 x capsule bytes (read + write), (1 + n) x for an n-way
+// fork.  Work decomposition: the byte ranges are cut into tiles of kCopyTileBytes (16 KiB)
+// numbered globally; CTA c handles tiles c, c + grid, ... (all tiles cost the same, so a
+// static round-robin is balanced).  A tile is moved with 16-byte vector loads/stores, all
+// loads of a thread issued before its first store (kCopyUnroll x 16 B in flight per thread,
+// 8 CTAs x 256 threads per SM -> 128 KiB in flight per SM, above the ~40 KiB that
+// latency x bandwidth per SM needs).  Odd tails and unaligned pointers take a byte path.
+#include "esc_internal.h"
+
+namespace esc {
+
+constexpr int kCopyBlocksPerSM = 8;
+
+__device__ __forceinline__ uint4 ld_stream(const uint4* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+                 "r"(v.w)
+                 : "memory");
+}
+
+// entry index of a global tile number: largest i with tile_begin[i] <= tile (zero-tile entries skipped)
+__device__ __forceinline__ uint32_t find_entry(const uint32_t* tile_begin, uint32_t n_seg, uint32_t tile) {
+    uint32_t lo = 0, hi = n_seg;  // invariant: tile_begin[lo] <= tile < tile_begin[hi]
+    while (hi - lo > 1) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (tile_begin[mid] <= tile) lo = mid;
+        else hi = mid;
+    }
+    return lo;
+}
+
+template <int kDst>
+__device__ __forceinline__ void copy_tile(const uint8_t* __restrict__ src, uint8_t* const* dst, uint32_t n_dst,
+                                          uint64_t n) {
+    const uint32_t tid = threadIdx.x;
+    bool aligned = (((uintptr_t)src) & 15u) == 0;
+#pragma unroll
+    for (int d = 0; d < kDst; ++d)
+        if (d < (int)n_dst) aligned = aligned && ((((uintptr_t)dst[d]) & 15u) == 0);
+    if (aligned) {
+        const uint4* s = (const uint4*)src;
+        if (n == kCopyTileBytes) {  // full tile: all loads first, then all stores
+            uint4 v[kCopyUnroll];
+#pragma unroll
+            for (int u = 0; u < (int)kCopyUnroll; ++u) v[u] = ld_stream(s + tid + u * kCopyThreads);
+#pragma unroll
+            for (int d = 0; d < kDst; ++d) {
+                if (d < (int)n_dst) {
+                    uint4* o = (uint4*)dst[d];
+#pragma unroll
+                    for (int u = 0; u < (int)kCopyUnroll; ++u) st_stream(o + tid + u * kCopyThreads, v[u]);
+                }
+            }
+            return;
+        }
+        const uint32_t n16 = (uint32_t)(n >> 4);
+        for (uint32_t i = tid; i < n16; i += kCopyThreads) {
+            const uint4 v = ld_stream(s + i);
+#pragma unroll
+            for (int d = 0; d < kDst; ++d)
+                if (d < (int)n_dst) st_stream((uint4*)dst[d] + i, v);
+        }
+        for (uint32_t i = (n16 << 4) + tid; i < n; i += kCopyThreads) {
+            const uint8_t b = src[i];
+#pragma unroll
+            for (int d = 0; d < kDst; ++d)
+                if (d < (int)n_dst) dst[d][i] = b;
+        }
+        return;
+    }
+    for (uint32_t i = tid; i < n; i += kCopyThreads) {  // byte path: exact for any alignment
+        const uint8_t b = src[i];
+#pragma unroll
+        for (int d = 0; d < kDst; ++d)
+            if (d < (int)n_dst) dst[d][i] = b;
+    }
+}
+
+__device__ __forceinline__ void copy_body(const CopyTable& t) {
+    const uint32_t n_tiles = t.n_tiles, n_seg = t.n_seg;
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const uint32_t e = find_entry(t.tile_begin, n_seg, tile);
+        const uint64_t off = (uint64_t)(tile - t.tile_begin[e]) * kCopyTileBytes;
+        const uint64_t left = t.bytes[e] - off;
+        uint8_t* d = t.dst[e] + off;
+        copy_tile<1>(t.src[e] + off, &d, 1, left < kCopyTileBytes ? left : kCopyTileBytes);
+    }
+}
+
+// table in kernel-parameter space: no H2D copy, no device allocation per verb
+__global__ void __launch_bounds__(kCopyThreads, kCopyBlocksPerSM) esc_copy_kernel(const __grid_constant__ CopyTable t) {
+    copy_body(t);
+}
+
+// table in global memory: the restore node of a captured graph (PAPER.md:110,128 — the host
+// overwrites the bound table between replays; the graph is never recaptured)
+__global__ void __launch_bounds__(kCopyThreads, kCopyBlocksPerSM) esc_copy_indirect_kernel(const CopyTable* __restrict__ tp) {
+    copy_body(*tp);
+}
+
+// fork: read each tile once, write it to n_dst live sets
+__global__ void __launch_bounds__(kCopyThreads, kCopyBlocksPerSM) esc_fork_kernel(const __grid_constant__ ForkTable t) {
+    const uint32_t n_tiles = t.n_tiles, n_seg = t.n_seg, n_dst = t.n_dst;
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const uint32_t e = find_entry(t.tile_begin, n_seg, tile);
+        const uint64_t off = (uint64_t)(tile - t.tile_begin[e]) * kCopyTileBytes;
+        const uint64_t left = t.bytes[e] - off;
+        uint8_t* d[ESC_MAX_FORK];
+#pragma unroll
+        for (int i = 0; i < (int)ESC_MAX_FORK; ++i) d[i] = i < (int)n_dst ? t.dst[i][e] + off : nullptr;
+        copy_tile<ESC_MAX_FORK>(t.src[e] + off, d, n_dst, left < kCopyTileBytes ? left : kCopyTileBytes);
+    }
+}
+
+// ---- host -----------------------------------------------------------------------------------
+int copy_grid_blocks(const esc_ctx* ctx) { return ctx->sm_count * kCopyBlocksPerSM; }
+
+static uint32_t fill_tiles(uint32_t* tile_begin, const uint64_t* bytes, uint32_t n) {
+    uint64_t t = 0;
+    for (uint32_t i = 0; i < n; ++i) {
+        tile_begin[i] = (uint32_t)t;
+        t += (bytes[i] + kCopyTileBytes - 1) / kCopyTileBytes;
+    }
+    tile_begin[n] = (uint32_t)t;
+    return (uint32_t)t;
+}
+
+void build_copy_table(CopyTable* t, const uint8_t* const* src, uint8_t* const* dst, const uint64_t* bytes, uint32_t n) {
+    memset(t, 0, sizeof *t);
+    t->n_seg = n;
+    t->n_tiles = fill_tiles(t->tile_begin, bytes, n);
+    for (uint32_t i = 0; i < n; ++i) {
+        t->src[i] = src[i];
+        t->dst[i] = dst[i];
+        t->bytes[i] = bytes[i];
+    }
+}
+
+static uint32_t pick_grid(const esc_ctx* ctx, uint32_t n_tiles) {
+    const uint32_t cap = (uint32_t)copy_grid_blocks(ctx);
+    return n_tiles < cap ? n_tiles : cap;
+}
+
+int launch_copy(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* dst, const uint64_t* bytes, uint32_t n,
+                cudaStream_t stream) {
+    for (uint32_t first = 0; first < n; first += kCopyMaxSeg) {
+        const uint32_t m = n - first < kCopyMaxSeg ? n - first : kCopyMaxSeg;
+        CopyTable t;
+        build_copy_table(&t, src + first, dst + first, bytes + first, m);
+        if (t.n_tiles == 0) continue;
+        esc_copy_kernel<<<pick_grid(ctx, t.n_tiles), kCopyThreads, 0, stream>>>(t);
+        ESC_CUDA(cudaGetLastError());
+    }
+    return ESC_OK;
+}
+
+int launch_copy_indirect(const esc_ctx* ctx, const CopyTable* table_dev, uint32_t grid_blocks, cudaStream_t stream) {
+    (void)ctx;
+    esc_copy_indirect_kernel<<<grid_blocks, kCopyThreads, 0, stream>>>(table_dev);
+    ESC_CUDA(cudaGetLastError());
+    return ESC_OK;
+}
+
+int launch_fork(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* const* dst, uint32_t n_dst,
+                const uint64_t* bytes, uint32_t n, cudaStream_t stream) {
+    for (uint32_t first = 0; first < n; first += kCopyMaxSegFork) {
+        const uint32_t m = n - first < kCopyMaxSegFork ? n - first : kCopyMaxSegFork;
+        ForkTable t;
+        memset(&t, 0, sizeof t);
+        t.n_seg = m;
+        t.n_dst = n_dst;
+        t.n_tiles = fill_tiles(t.tile_begin, bytes + first, m);
+        for (uint32_t i = 0; i < m; ++i) {
+            t.src[i] = src[first + i];
+            t.bytes[i] = bytes[first + i];
+            for (uint32_t d = 0; d < n_dst; ++d) t.dst[d][i] = dst[d][first + i];
+        }
+        if (t.n_tiles == 0) continue;
+        esc_fork_kernel<<<pick_grid(ctx, t.n_tiles), kCopyThreads, 0, stream>>>(t);
+        ESC_CUDA(cudaGetLastError());
+    }
+    return ESC_OK;
+}
+
+}  // namespace esc

@@ -1,0 +1,116 @@
+// Internal structures of libesc (host side) + the device copy-table layout.
+// The public contract is include/esc.h; nothing here crosses the ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "esc.h"
+
+namespace esc {
+
+// ---- error plumbing -------------------------------------------------------------------
+extern thread_local int g_last_cuda_error;
+inline int cuda_fail(cudaError_t e) {
+    g_last_cuda_error = (int)e;
+    return ESC_ERR_CUDA;
+}
+#define ESC_CUDA(call)                                        \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return ::esc::cuda_fail(e__); \
+    } while (0)
+
+// ---- copy table (what the capsule copy kernel consumes) --------------------------------
+// One entry per (row, segment): `bytes` valid bytes from src to dst[0..n_dst).
+// Tiles of kCopyTileBytes are numbered globally; tile_begin[i] is the first tile of entry i.
+constexpr uint32_t kCopyThreads = 256;
+constexpr uint32_t kCopyUnroll = 4;                    // 16-byte vectors in flight per thread
+constexpr uint32_t kCopyTileBytes = kCopyThreads * kCopyUnroll * 16u;   // 16 KiB
+constexpr uint32_t kCopyMaxSeg = 112;                 // entries per launch (table <= 4 KiB kernel params)
+constexpr uint32_t kCopyMaxSegFork = 96;              // entries per fork launch
+
+struct CopyTable {                                    // single destination: 3600 B
+    uint32_t n_seg;
+    uint32_t n_tiles;
+    uint32_t tile_begin[kCopyMaxSeg + 1];
+    uint32_t pad_;
+    const uint8_t* src[kCopyMaxSeg];
+    uint8_t* dst[kCopyMaxSeg];
+    uint64_t bytes[kCopyMaxSeg];
+};
+
+struct ForkTable {                                    // n_dst destinations (large kernel params)
+    uint32_t n_seg;
+    uint32_t n_tiles;
+    uint32_t n_dst;
+    uint32_t pad_;
+    uint32_t tile_begin[kCopyMaxSegFork + 1];
+    uint32_t pad2_;
+    const uint8_t* src[kCopyMaxSegFork];
+    uint64_t bytes[kCopyMaxSegFork];
+    uint8_t* dst[ESC_MAX_FORK][kCopyMaxSegFork];
+};
+
+// ---- handles ----------------------------------------------------------------------------
+struct Row {
+    std::string name;
+    uint8_t* base;
+    uint64_t capacity, fixed_bytes, bytes_per_token, seg_stride;
+    uint32_t n_seg;
+};
+
+}  // namespace esc
+
+struct esc_ctx {
+    int device;
+    int sm_count;
+    int l2_bytes;
+};
+
+struct esc_bufset {
+    esc_ctx* ctx;
+    bool frozen;                      // false: live set; true: capsule
+    std::vector<esc::Row> rows;       // live: the registered buffers.  capsule: layout copy (base = nullptr)
+    uint64_t layout_digest;
+    uint64_t position;                // live: current token position; capsule: boundary P'
+    // capsule only
+    uint8_t* slab;
+    uint64_t slab_bytes, payload_bytes, chunk, prefix_digest;
+};
+
+namespace esc {
+
+struct Seg {                          // host-side flattened (row, segment) of a live<->slab pairing
+    uint8_t* live;
+    uint64_t slab_off;
+    uint64_t bytes;
+};
+
+uint64_t seg_valid(const Row& r, uint64_t P);
+int check_fit(const std::vector<Row>& rows, uint64_t P);
+// slab layout walk: fills segs (live pointers relative to `rows`), returns slab bytes / payload
+void layout_walk(const std::vector<Row>& rows, uint64_t P, std::vector<Seg>* segs, uint64_t* slab_bytes,
+                 uint64_t* payload_bytes);
+
+// copy kernel launchers (copy_kernel.cu)
+int copy_grid_blocks(const esc_ctx* ctx);
+// Launch the copy of `n` (src,dst,bytes) entries, splitting into several launches only when n > kCopyMaxSeg.
+int launch_copy(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* dst, const uint64_t* bytes, uint32_t n,
+                cudaStream_t stream);
+int launch_fork(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* const* dst, uint32_t n_dst,
+                const uint64_t* bytes, uint32_t n, cudaStream_t stream);
+// table-in-global-memory variant used inside captured graphs
+void build_copy_table(CopyTable* t, const uint8_t* const* src, uint8_t* const* dst, const uint64_t* bytes, uint32_t n);
+int launch_copy_indirect(const esc_ctx* ctx, const CopyTable* table_dev, uint32_t grid_blocks, cudaStream_t stream);
+
+// scan (scan_kernel.cu)
+struct ScanShape {
+    uint32_t B, H, dk, dv, in_dtype, out_dtype, chunk;
+};
+bool decode_key(esc_shape_key key, ScanShape* s);
+int launch_scan(const esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g,
+                const float* state_in, float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream);
+
+}  // namespace esc

@@ -1,0 +1,153 @@
+// Captured replay plan: [restore node] -> [scan node per layer] as ONE CUDA graph
+// (include/esc.h: esc_graph_*).  PAPER.md:128-129: restore "replay[s] the already-captured
+// Graph[key] — never a recapture"; the host overwrites a bound sub-buffer between
+// replays.  Here the bound sub-buffer is the restore node's copy table: it lives in device
+// memory owned by the graph, so binding another capsule is one small async H2D copy and the
+// graph's kernel nodes (pointers, grids) never change.
+#include <new>
+
+#include "esc_internal.h"
+
+struct esc_graph {
+    esc_ctx* ctx;
+    esc_bufset* live;             // NULL: cold plan (no restore node)
+    cudaGraph_t graph;
+    cudaGraphExec_t exec;
+    esc::CopyTable* table_dev;    // device-resident "current capsule" table
+    esc::CopyTable* table_host;   // pinned mirror
+    cudaEvent_t table_copied;     // guards reuse of the pinned mirror
+    bool bound;
+    uint64_t bound_boundary;
+};
+
+using namespace esc;
+
+static void graph_free(esc_graph* g) {
+    if (!g) return;
+    if (g->exec) cudaGraphExecDestroy(g->exec);
+    if (g->graph) cudaGraphDestroy(g->graph);
+    if (g->table_dev) cudaFree(g->table_dev);
+    if (g->table_host) cudaFreeHost(g->table_host);
+    if (g->table_copied) cudaEventDestroy(g->table_copied);
+    delete g;
+}
+
+extern "C" {
+
+int esc_graph_capture(esc_ctx* ctx, esc_bufset* live, uint64_t max_boundary, const esc_scan_args* layers,
+                      uint32_t n_layers, void* stream, esc_graph** out_graph) {
+    if (!ctx || !out_graph || (n_layers && !layers) || (!live && n_layers == 0)) return ESC_ERR_INVALID;
+    if (!stream) return ESC_ERR_INVALID;  // the legacy default stream cannot be captured
+    if (live && live->frozen) return ESC_ERR_INVALID;
+    uint32_t grid = 0;
+    if (live) {
+        int rc = check_fit(live->rows, max_boundary);
+        if (rc != ESC_OK) return rc;
+        std::vector<Seg> segs;
+        layout_walk(live->rows, max_boundary, &segs, nullptr, nullptr);
+        if (segs.size() > kCopyMaxSeg) return ESC_ERR_UNSUPPORTED;
+        uint64_t tiles = 0;
+        for (const Seg& s : segs) tiles += (s.bytes + kCopyTileBytes - 1) / kCopyTileBytes;
+        const uint64_t cap = (uint64_t)copy_grid_blocks(ctx);
+        grid = (uint32_t)(tiles < cap ? (tiles ? tiles : 1) : cap);
+    }
+    // validate the scan layers and set kernel attributes BEFORE the capture begins
+    std::vector<ScanShape> shapes(n_layers);
+    for (uint32_t i = 0; i < n_layers; ++i) {
+        const esc_scan_args& a = layers[i];
+        if (!decode_key(a.key, &shapes[i]) || !a.state_out || a.reserved != 0) return ESC_ERR_INVALID;
+        if (a.T > 0 && (!a.q || !a.k || !a.v || !a.g || !a.o)) return ESC_ERR_INVALID;
+        if (a.chunk != shapes[i].chunk) return ESC_ERR_MISMATCH;
+        if (a.t_stride < a.T) return ESC_ERR_INVALID;
+        const uintptr_t all = (uintptr_t)a.q | (uintptr_t)a.k | (uintptr_t)a.v | (uintptr_t)a.state_in |
+                              (uintptr_t)a.state_out | (uintptr_t)a.o;
+        if ((all & 15u) || ((uintptr_t)a.g & 3u)) return ESC_ERR_UNALIGNED;
+        int rc = launch_scan(ctx, shapes[i], nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, nullptr);
+        if (rc != ESC_OK) return rc;
+    }
+
+    esc_graph* g = new (std::nothrow) esc_graph();
+    if (!g) return ESC_ERR_INVALID;
+    g->ctx = ctx;
+    g->live = live;
+    g->bound = false;
+    cudaError_t e = cudaSuccess;
+    if (live) {
+        e = cudaMalloc((void**)&g->table_dev, sizeof(CopyTable));
+        if (e == cudaSuccess) e = cudaMallocHost((void**)&g->table_host, sizeof(CopyTable));
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->table_copied, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaMemset(g->table_dev, 0, sizeof(CopyTable));  // n_tiles = 0: a no-op until bound
+        if (e != cudaSuccess) {
+            graph_free(g);
+            return cuda_fail(e);
+        }
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    e = cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) {
+        graph_free(g);
+        return cuda_fail(e);
+    }
+    int rc = ESC_OK;
+    if (live) rc = launch_copy_indirect(ctx, g->table_dev, grid, st);
+    for (uint32_t i = 0; i < n_layers && rc == ESC_OK; ++i) {
+        const esc_scan_args& a = layers[i];
+        rc = launch_scan(ctx, shapes[i], a.q, a.k, a.v, a.g, a.state_in, a.state_out, a.o, a.T, a.t_stride, st);
+    }
+    e = cudaStreamEndCapture(st, &g->graph);
+    if (rc != ESC_OK || e != cudaSuccess) {
+        graph_free(g);
+        return rc != ESC_OK ? rc : cuda_fail(e);
+    }
+    e = cudaGraphInstantiate(&g->exec, g->graph, 0);
+    if (e != cudaSuccess) {
+        graph_free(g);
+        return cuda_fail(e);
+    }
+    *out_graph = g;
+    return ESC_OK;
+}
+
+int esc_graph_set_capsule(esc_graph* graph, const esc_bufset* capsule, void* stream) {
+    if (!graph || !graph->live || !capsule || !capsule->frozen) return ESC_ERR_INVALID;
+    esc_bufset* live = graph->live;
+    if (live->layout_digest != capsule->layout_digest || live->rows.size() != capsule->rows.size())
+        return ESC_ERR_MISMATCH;
+    int rc = check_fit(live->rows, capsule->position);
+    if (rc != ESC_OK) return rc;
+    std::vector<Seg> segs;
+    layout_walk(live->rows, capsule->position, &segs, nullptr, nullptr);
+    if (segs.size() > kCopyMaxSeg) return ESC_ERR_UNSUPPORTED;
+    std::vector<const uint8_t*> src(segs.size());
+    std::vector<uint8_t*> dst(segs.size());
+    std::vector<uint64_t> bytes(segs.size());
+    for (size_t i = 0; i < segs.size(); ++i) {
+        src[i] = capsule->slab + segs[i].slab_off;
+        dst[i] = segs[i].live;
+        bytes[i] = segs[i].bytes;
+    }
+    ESC_CUDA(cudaEventSynchronize(graph->table_copied));  // previous upload has left the pinned mirror
+    build_copy_table(graph->table_host, src.data(), dst.data(), bytes.data(), (uint32_t)segs.size());
+    ESC_CUDA(cudaMemcpyAsync(graph->table_dev, graph->table_host, sizeof(CopyTable), cudaMemcpyHostToDevice,
+                             (cudaStream_t)stream));
+    ESC_CUDA(cudaEventRecord(graph->table_copied, (cudaStream_t)stream));
+    graph->bound = true;
+    graph->bound_boundary = capsule->position;
+    return ESC_OK;
+}
+
+int esc_graph_launch(esc_graph* graph, void* stream) {
+    if (!graph) return ESC_ERR_INVALID;
+    if (graph->live && !graph->bound) return ESC_ERR_INVALID;
+    ESC_CUDA(cudaGraphLaunch(graph->exec, (cudaStream_t)stream));
+    if (graph->live) graph->live->position = graph->bound_boundary;
+    return ESC_OK;
+}
+
+int esc_graph_destroy(esc_graph* graph) {
+    if (!graph) return ESC_ERR_INVALID;
+    graph_free(graph);
+    return ESC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,259 @@
+"""ctypes binding of libesc.so — the C ABI declared in include/esc.h, same names.
+
+Argument marshalling only: every step of the path (copy, scan, graph) runs in the library's
+CUDA kernels.  torch is used by callers for device memory and streams; this module accepts
+either torch tensors (their data_ptr()) or raw integer device addresses.  There is no CPU
+fallback: if libesc.so is missing, importing this module raises.
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libesc.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        "libesc.so is not built (%s). Run `python -m paper_2606_20537_b200.build` "
+        "(nvcc, sm_100a). There is no CPU fallback." % LIB_PATH)
+
+lib = C.CDLL(LIB_PATH)
+
+OK, ERR_INVALID, ERR_UNALIGNED, ERR_MISMATCH, ERR_CAPACITY, ERR_UNSUPPORTED, ERR_CUDA = 0, -1, -2, -3, -4, -5, -6
+DTYPE_BF16, DTYPE_F32 = 1, 2
+SNAPSHOT_ALLOW_UNALIGNED = 1
+MAX_FORK = 16
+MAX_ROWS = 256
+POSITION_UNKNOWN = 2**64 - 1
+
+
+class EscError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        msg = lib.esc_strerror(code).decode()
+        if code == ERR_CUDA:
+            msg += " (cudaError %d)" % lib.esc_last_cuda_error()
+        super().__init__("%s: %s" % (where, msg))
+
+
+class BufDesc(C.Structure):
+    _fields_ = [("name", C.c_char_p), ("dev_ptr", C.c_void_p), ("capacity_bytes", C.c_uint64),
+                ("fixed_bytes", C.c_uint64), ("bytes_per_token", C.c_uint64), ("n_seg", C.c_uint32),
+                ("reserved", C.c_uint32), ("seg_stride", C.c_uint64)]
+
+
+class CapsuleInfo(C.Structure):
+    _fields_ = [("boundary", C.c_uint64), ("chunk", C.c_uint64), ("slab_bytes", C.c_uint64),
+                ("payload_bytes", C.c_uint64), ("layout_digest", C.c_uint64), ("prefix_digest", C.c_uint64),
+                ("n_rows", C.c_uint32), ("n_segments", C.c_uint32), ("aligned", C.c_uint32), ("reserved", C.c_uint32)]
+
+
+class ScanArgs(C.Structure):
+    _fields_ = [("key", C.c_uint64), ("q", C.c_void_p), ("k", C.c_void_p), ("v", C.c_void_p), ("g", C.c_void_p),
+                ("state_in", C.c_void_p), ("state_out", C.c_void_p), ("o", C.c_void_p),
+                ("T", C.c_uint64), ("t_stride", C.c_uint64), ("chunk", C.c_uint32), ("reserved", C.c_uint32)]
+
+
+_P = C.c_void_p
+_sig = {
+    "esc_strerror": (C.c_char_p, [C.c_int]),
+    "esc_abi_version": (C.c_uint32, []),
+    "esc_last_cuda_error": (C.c_int, []),
+    "esc_ctx_create": (C.c_int, [C.c_int, C.POINTER(_P)]),
+    "esc_ctx_destroy": (C.c_int, [_P]),
+    "esc_ctx_sm_count": (C.c_int, [_P, C.POINTER(C.c_int)]),
+    "esc_bufset_create": (C.c_int, [_P, C.POINTER(BufDesc), C.c_uint32, C.POINTER(_P)]),
+    "esc_bufset_destroy": (C.c_int, [_P]),
+    "esc_bufset_layout_digest": (C.c_int, [_P, C.POINTER(C.c_uint64)]),
+    "esc_bufset_set_position": (C.c_int, [_P, C.c_uint64]),
+    "esc_bufset_get_position": (C.c_int, [_P, C.POINTER(C.c_uint64)]),
+    "esc_capsule_bytes": (C.c_int, [_P, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]),
+    "esc_align_boundary": (C.c_uint64, [C.c_uint64, C.c_uint64]),
+    "esc_snapshot": (C.c_int, [_P, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, _P, C.c_uint64, _P, C.POINTER(_P)]),
+    "esc_restore": (C.c_int, [_P, _P, C.POINTER(C.c_uint64), _P]),
+    "esc_fork": (C.c_int, [_P, C.POINTER(_P), C.c_uint32, _P]),
+    "esc_rollback": (C.c_int, [_P, _P, _P]),
+    "esc_capsule_info_get": (C.c_int, [_P, C.POINTER(CapsuleInfo)]),
+    "esc_capsule_valid_end": (C.c_int, [_P, C.c_uint32, C.POINTER(C.c_uint64)]),
+    "esc_shape_key_make": (C.c_uint64, [C.c_uint32] * 7),
+    "esc_linattn_scan": (C.c_int, [_P, C.c_uint64] + [_P] * 7 + [C.c_uint64, C.c_uint64, C.c_uint32, _P]),
+    "esc_graph_capture": (C.c_int, [_P, _P, C.c_uint64, C.POINTER(ScanArgs), C.c_uint32, _P, C.POINTER(_P)]),
+    "esc_graph_set_capsule": (C.c_int, [_P, _P, _P]),
+    "esc_graph_launch": (C.c_int, [_P, _P]),
+    "esc_graph_destroy": (C.c_int, [_P]),
+}
+for _n, (_r, _a) in _sig.items():
+    _f = getattr(lib, _n)
+    _f.restype, _f.argtypes = _r, _a
+EXPORTS = tuple(_sig)
+
+
+def _check(rc, where):
+    if rc != OK:
+        raise EscError(rc, where)
+
+
+def _ptr(x):
+    """torch tensor / int / None -> device address (int or None)."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    return x.data_ptr()
+
+
+def _stream(s):
+    """torch.cuda.Stream / int / None -> cudaStream_t value."""
+    if s is None:
+        return None
+    if isinstance(s, int):
+        return s or None
+    return s.cuda_stream or None
+
+
+def strerror(code):
+    return lib.esc_strerror(code).decode()
+
+
+def abi_version():
+    return int(lib.esc_abi_version())
+
+
+def align_boundary(P, chunk):
+    return int(lib.esc_align_boundary(P, chunk))
+
+
+def shape_key_make(B, H, d_k, d_v, in_dtype=DTYPE_BF16, out_dtype=DTYPE_F32, chunk=64):
+    return int(lib.esc_shape_key_make(B, H, d_k, d_v, in_dtype, out_dtype, chunk))
+
+
+class Ctx:
+    def __init__(self, device=0):
+        h = _P()
+        _check(lib.esc_ctx_create(device, C.byref(h)), "esc_ctx_create")
+        self.h = h
+
+    @property
+    def sm_count(self):
+        n = C.c_int()
+        _check(lib.esc_ctx_sm_count(self.h, C.byref(n)), "esc_ctx_sm_count")
+        return n.value
+
+    def close(self):
+        if self.h:
+            lib.esc_ctx_destroy(self.h)
+            self.h = None
+
+
+class BufSet:
+    """A live set (esc_bufset_create) or a capsule (returned by snapshot)."""
+
+    def __init__(self, handle, keep=()):
+        self.h = handle
+        self._keep = keep   # python references that must outlive the handle (tensors, slab)
+
+    @property
+    def layout_digest(self):
+        d = C.c_uint64()
+        _check(lib.esc_bufset_layout_digest(self.h, C.byref(d)), "esc_bufset_layout_digest")
+        return d.value
+
+    @property
+    def position(self):
+        p = C.c_uint64()
+        _check(lib.esc_bufset_get_position(self.h, C.byref(p)), "esc_bufset_get_position")
+        return p.value
+
+    def set_position(self, P):
+        _check(lib.esc_bufset_set_position(self.h, P), "esc_bufset_set_position")
+
+    def capsule_bytes(self, P):
+        a, b = C.c_uint64(), C.c_uint64()
+        _check(lib.esc_capsule_bytes(self.h, P, C.byref(a), C.byref(b)), "esc_capsule_bytes")
+        return a.value, b.value
+
+    def info(self):
+        i = CapsuleInfo()
+        _check(lib.esc_capsule_info_get(self.h, C.byref(i)), "esc_capsule_info_get")
+        return i
+
+    def valid_end(self, row):
+        n = C.c_uint64()
+        _check(lib.esc_capsule_valid_end(self.h, row, C.byref(n)), "esc_capsule_valid_end")
+        return n.value
+
+    def destroy(self):
+        if self.h:
+            lib.esc_bufset_destroy(self.h)
+            self.h = None
+            self._keep = ()
+
+
+def bufset_create(ctx, rows):
+    """rows: iterable of (name, tensor_or_addr, capacity_bytes, fixed_bytes, bytes_per_token, n_seg, seg_stride)."""
+    rows = list(rows)
+    arr = (BufDesc * len(rows))()
+    for i, (name, buf, cap, fixed, per_tok, n_seg, stride) in enumerate(rows):
+        arr[i] = BufDesc(name.encode(), _ptr(buf), cap, fixed, per_tok, n_seg, 0, stride)
+    h = _P()
+    _check(lib.esc_bufset_create(ctx.h, arr, len(rows), C.byref(h)), "esc_bufset_create")
+    return BufSet(h, keep=tuple(r[1] for r in rows))
+
+
+def snapshot(live, P, chunk, storage, storage_bytes=None, prefix_digest=0, flags=0, stream=None):
+    """storage: torch uint8 tensor (or address + storage_bytes). Returns the capsule BufSet."""
+    if storage_bytes is None:
+        storage_bytes = storage.numel() * storage.element_size()
+    h = _P()
+    _check(lib.esc_snapshot(live.h, P, chunk, prefix_digest, flags, _ptr(storage), storage_bytes, _stream(stream),
+                            C.byref(h)), "esc_snapshot")
+    return BufSet(h, keep=(storage,))
+
+
+def restore(live, capsule, expect_prefix_digest=None, stream=None):
+    e = None if expect_prefix_digest is None else C.byref(C.c_uint64(expect_prefix_digest))
+    _check(lib.esc_restore(live.h, capsule.h, e, _stream(stream)), "esc_restore")
+
+
+def fork(capsule, lives, stream=None):
+    arr = (_P * len(lives))(*[l.h for l in lives])
+    _check(lib.esc_fork(capsule.h, arr, len(lives), _stream(stream)), "esc_fork")
+
+
+def rollback(live, capsule_earlier, stream=None):
+    _check(lib.esc_rollback(live.h, capsule_earlier.h, _stream(stream)), "esc_rollback")
+
+
+def linattn_scan(ctx, key, q, k, v, g, state_in, state_out, o, T, t_stride, chunk, stream=None):
+    _check(lib.esc_linattn_scan(ctx.h, key, _ptr(q), _ptr(k), _ptr(v), _ptr(g), _ptr(state_in), _ptr(state_out),
+                                _ptr(o), T, t_stride, chunk, _stream(stream)), "esc_linattn_scan")
+
+
+def scan_args(key, q, k, v, g, state_in, state_out, o, T, t_stride, chunk):
+    return ScanArgs(key, _ptr(q), _ptr(k), _ptr(v), _ptr(g), _ptr(state_in), _ptr(state_out), _ptr(o),
+                    T, t_stride, chunk, 0)
+
+
+class Graph:
+    def __init__(self, handle, keep=()):
+        self.h = handle
+        self._keep = keep
+
+    def set_capsule(self, capsule, stream=None):
+        _check(lib.esc_graph_set_capsule(self.h, capsule.h, _stream(stream)), "esc_graph_set_capsule")
+
+    def launch(self, stream=None):
+        _check(lib.esc_graph_launch(self.h, _stream(stream)), "esc_graph_launch")
+
+    def destroy(self):
+        if self.h:
+            lib.esc_graph_destroy(self.h)
+            self.h = None
+
+
+def graph_capture(ctx, live, max_boundary, layers, stream):
+    """layers: list of ScanArgs; live may be None (cold plan).  stream must be a non-default stream."""
+    arr = (ScanArgs * max(1, len(layers)))(*layers)
+    h = _P()
+    _check(lib.esc_graph_capture(ctx.h, live.h if live is not None else None, max_boundary, arr, len(layers),
+                                 _stream(stream), C.byref(h)), "esc_graph_capture")
+    return Graph(h, keep=(live, tuple(layers)))
