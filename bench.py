@@ -1,0 +1,402 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the capsule + chunked-scan hot path on B200.
+
+Step (BASELINE.json configs[1], "Hybrid capsule, prefix 2k"): one pass of the whole hot path over one
+synthetic session —  snapshot(P=2048) of the 24-layer hybrid live set (66 MiB capsule)  ->  ONE CUDA graph
+[ restore(capsule) -> 18-layer suffix scan of 64 tokens, chunk 64 ].  Source / destination slabs rotate over
+a working set of capsules and L2 is flushed between timed steps (PAPER.md:301's 20-capsule working set is the
+model), so neither verb reads L2-resident bytes.
+
+  value  = capsule bytes moved by the verbs (snapshot r+w + restore r+w = 4 x capsule bytes) / step time, GB/s
+  e2e    = the same with the step's suffix inputs copied H2D from pinned memory and its outputs copied D2H
+           inside the timed region
+  extras = restore-alone GB/s, scan tokens/s at config 2's cold length, warm-vs-cold table at 2k-16k
+  --impl reference times the CPU oracle (oracle/) on the same step.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+P_STEP, SUFFIX, CHUNK = 2048, 64, 64
+N_LINEAR = 18
+METRIC = "capsule restore GB/s (% of HBM peak); scan tokens/s; warm-vs-cold rebuild ms @2k-16k"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="esc", choices=["esc", "reference"])
+    ap.add_argument("--no-extras", action="store_true", help="skip the scan / warm-vs-cold / cpu_baseline extras")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    """Roofline denominators: MEASURED_PEAKS.json (driver-written), else the profiling guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d.get("bf16_tflops", 1590.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1]))
+                mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out = {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                   "samples": len(sm)}
+        return out
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle, as it stands, on the same step
+# ------------------------------------------------------------------------------------------------
+def oracle_step_setup():
+    import numpy as np
+    import oracle
+    from paper_2606_20537_b200 import synth
+    specs = synth.hybrid_layout(P_STEP + SUFFIX)
+    host, lin = [], []
+    for i, s in enumerate(specs):
+        if ".lin." in s.name:
+            host.append(synth.scan_state(1, 16, 128, 128, seed_ids=(30, 0, i), scale=0.3).view(np.uint8).reshape(-1).copy())
+            lin.append(i)
+        else:
+            host.append(synth.random_bytes(s.capacity_bytes, 40, i))
+    rows = [oracle.CapsuleRow(s.name, h, s.fixed_bytes, s.bytes_per_token, s.n_seg, s.seg_stride)
+            for s, h in zip(specs, host)]
+    ins = [synth.scan_inputs(1, SUFFIX, 16, 128, 128, seed_ids=(31, 0, n)).as_f32() for n in range(len(lin))]
+    return oracle, np, rows, host, lin, ins
+
+
+def oracle_step(ctx):
+    """snapshot -> restore -> 18-layer suffix scan, all on the host (oracle/ only)."""
+    oracle, np, rows, host, lin, ins = ctx
+    slab = oracle.capsule_snapshot(rows, P_STEP)
+    oracle.capsule_restore(rows, P_STEP, slab)
+    for n, i in enumerate(lin):
+        s0 = host[i].view(np.float32).reshape(1, 16, 128, 128).astype(np.float64)
+        o, s = oracle.linattn_recurrence(*ins[n], s0)
+        host[i].view(np.float32)[:] = s.astype(np.float32).reshape(-1)
+    return slab.nbytes
+
+
+def time_oracle(steps, warmup):
+    ctx = oracle_step_setup()
+    payload = 0
+    for _ in range(warmup):
+        payload = oracle_step(ctx)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        payload = oracle_step(ctx)
+    dt = (time.perf_counter() - t0) / max(1, steps)
+    return dt, payload, ctx[0].max_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps = max(1, min(args.steps, 20))
+    dt, payload, cores = time_oracle(steps, max(1, min(args.warmup, 3)))
+    gbs = 4 * payload / dt / 1e9
+    sample = "full step: snapshot + restore of the 66 MiB capsule by memcpy + 18 x 64-token fp64 recurrence"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": gbs, "unit": "GB/s", "n_gpus": args.gpus, "steps": steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[1]: hybrid capsule prefix 2048, 66 MiB, snapshot+restore+18x64-token suffix scan",
+                   "prefix": P_STEP, "suffix": SUFFIX, "chunk": CHUNK},
+        "cpu_baseline": {"value": gbs, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gbs, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+# ------------------------------------------------------------------------------------------------
+# esc arm: the CUDA path through the C ABI
+# ------------------------------------------------------------------------------------------------
+ALG_BYTES_PER_TOKEN_HEAD = 2 * 128 + 2 * 128 + 2 * 128 + 4 + 4 * 128   # q,k,v bf16 + g fp32 + o fp32 = 1284 B (d=128)
+N_CAPSULES = 20           # resident working set the verbs rotate over
+FLUSH_BYTES = 512 << 20   # > 126 MB L2
+
+
+def _ev_ms(pairs):
+    return [a.elapsed_time(b) for a, b in pairs]
+
+
+def run_esc(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_20537_b200 import esc, workload   # raises if libesc.so is missing: no fallback
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    pk = peaks()
+    ctx = esc.Ctx(local)
+    stream = torch.cuda.Stream()
+    sess = workload.HybridSession(ctx, P_STEP + SUFFIX, seed=rank, device=dev)
+    slab_bytes, payload = sess.capsule_bytes(P_STEP)
+    inputs = workload.SuffixInputs(N_LINEAR, SUFFIX, seed=rank, device=dev, pinned=True)
+    layers, key = workload.scan_layers(sess, inputs, CHUNK)
+    graph = esc.graph_capture(ctx, sess.set, P_STEP, layers, stream)
+    slabs = [sess.new_slab(P_STEP) for _ in range(N_CAPSULES)]
+    caps = [esc.snapshot(sess.set, P_STEP, CHUNK, s, stream=stream) for s in slabs]
+    flush = torch.empty(FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    stream.synchronize()
+    launches = [0]
+
+    def flush_l2():
+        with torch.cuda.stream(stream):
+            flush.fill_(1)
+
+    def step(i):
+        """snapshot(P) -> ONE graph launch [restore -> 18-layer suffix scan]."""
+        j = i % N_CAPSULES
+        sess.set.set_position(P_STEP)
+        caps[j].destroy()
+        caps[j] = esc.snapshot(sess.set, P_STEP, CHUNK, slabs[j], stream=stream)
+        graph.set_capsule(caps[(j + N_CAPSULES // 2) % N_CAPSULES], stream)   # written 10 steps ago: not in L2
+        graph.launch(stream)
+        launches[0] += 2 + N_LINEAR
+
+    def timed(fn, n, with_flush=True):
+        pairs = []
+        for i in range(n):
+            if with_flush:
+                flush_l2()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn(i)
+            b.record(stream)
+            pairs.append((a, b))
+        stream.synchronize()
+        return _ev_ms(pairs)
+
+    # ---- warm-up, then the timed region: EXACTLY K steps between barrier+sync ----------------------
+    timed(step, max(args.warmup, 3))
+    barrier()
+    sampler = ClockSampler(local)
+    launches[0] = 0
+    t_wall = time.perf_counter()
+    ms = timed(step, args.steps)
+    barrier()
+    wall_ms = (time.perf_counter() - t_wall) * 1e3
+    n_launch = launches[0]
+    ms_step = sum(ms) / len(ms)
+
+    # ---- end to end: suffix inputs H2D from pinned memory + outputs D2H inside the timed region -------
+    def step_e2e(i):
+        with torch.cuda.stream(stream):
+            inputs.h2d()
+        step(i)
+        with torch.cuda.stream(stream):
+            inputs.d2h()
+    timed(step_e2e, 3)
+    ms_e2e_l = timed(step_e2e, args.steps)
+    ms_e2e = sum(ms_e2e_l) / len(ms_e2e_l)
+
+    # ---- per-kernel durations (CUDA events on the launching stream, L2 flushed before each) ------------
+    def only_restore(i):
+        esc.restore(sess.set, caps[i % N_CAPSULES], stream=stream)
+
+    def only_snapshot(i):
+        j = i % N_CAPSULES
+        sess.set.set_position(P_STEP)
+        caps[j].destroy()
+        caps[j] = esc.snapshot(sess.set, P_STEP, CHUNK, slabs[j], stream=stream)
+
+    def only_suffix_scans(i):
+        for n in range(N_LINEAR):
+            q, k, v, g = inputs.dev[n]
+            esc.linattn_scan(ctx, key, q, k, v, g, sess.states[n], sess.states[n], inputs.out[n], SUFFIX, SUFFIX, CHUNK,
+                             stream=stream)
+    timed(only_restore, 3)
+    ms_restore = statistics.median(timed(only_restore, max(args.steps, 15)))
+    ms_snapshot = statistics.median(timed(only_snapshot, max(args.steps, 15)))
+    timed(only_suffix_scans, 3)
+    ms_suffix = statistics.median(timed(only_suffix_scans, max(args.steps, 15)))
+    clocks = sampler.stop()
+
+    # max over ranks
+    if world > 1:
+        t = torch.tensor([ms_step, ms_e2e, wall_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step, ms_e2e, wall_ms = t.tolist()
+    moved = 4 * payload                                  # snapshot r+w + restore r+w
+    value = world * moved / (ms_step * 1e-3) / 1e9
+    e2e_value = world * moved / (ms_e2e * 1e-3) / 1e9
+
+    copy_gbs = 2 * payload / (ms_restore * 1e-3) / 1e9
+    roof_copy = {"kernel": "esc_copy_kernel (restore, 66 MiB capsule, 30 segments)", "bound": "hbm",
+                 "achieved": copy_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": copy_gbs / pk["hbm_gbs"],
+                 "peak_source": pk["source"], "traffic": None, "us_per_launch": ms_restore * 1e3,
+                 "alg_bytes_per_launch": 2 * payload}
+    out = {
+        "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": "configs[1]: hybrid capsule prefix 2048 (18 fp32 fold states 16x128x128 + 6 layers bf16 KV), "
+                               "step = snapshot + ONE graph [restore + 18-layer 64-token suffix scan, chunk 64]",
+                   "prefix": P_STEP, "suffix": SUFFIX, "chunk": CHUNK, "capsule_bytes": payload,
+                   "capsule_segments": caps[0].info().n_segments, "working_set_capsules": N_CAPSULES,
+                   "l2": "flushed between timed steps (512 MiB fill) + capsules rotate over a 20-slab working set",
+                   "value_definition": "4 x capsule bytes (snapshot r+w, restore r+w) / step time, all ranks"},
+        "clocks": clocks, "gpu_launches": n_launch, "wall_ms_timed_region": wall_ms,
+        "e2e": {"value": e2e_value, "unit": "GB/s", "h2d_bytes_per_step": inputs.h2d_bytes(),
+                "d2h_bytes_per_step": inputs.d2h_bytes(), "ms_per_step": ms_e2e},
+        "breakdown_us": {"snapshot": ms_snapshot * 1e3, "restore": ms_restore * 1e3,
+                         "suffix_scan_18_layers": ms_suffix * 1e3, "step": ms_step * 1e3},
+        "restore": {"us": ms_restore * 1e3, "GBps": copy_gbs, "frac_of_measured_peak": copy_gbs / pk["hbm_gbs"],
+                    "frac_of_8TBps": copy_gbs / 8000.0},
+        "roofline": roof_copy,
+    }
+    if rank == 0 and world == 1 and not args.no_extras:
+        out.update(extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev))
+        if ms_suffix > ms_restore + ms_snapshot and "roofline_scan" in out:
+            out["roofline_dominant_in_step"] = "scan (suffix scans take %.0f us of the %.0f us step)" % (
+                ms_suffix * 1e3, ms_step * 1e3)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.no_extras:
+        dt, pl, cores = time_oracle(3, 1)
+        out["cpu_baseline"] = {"value": 4 * pl / dt / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle",
+                               "sample": "3 full steps (snapshot + restore of the 66 MiB capsule by memcpy + 18 x 64-token "
+                                         "fp64 recurrence), %.0f ms each" % (dt * 1e3)}
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
+    """Rank-0, N=1 extras: scan tokens/s + roofline at config 2's cold length, warm-vs-cold table at 2k-16k."""
+    res = {}
+    t_max = 16384 + SUFFIX
+    sess = workload.HybridSession(ctx, t_max, seed=7, device=dev)
+    suffix = workload.SuffixInputs(N_LINEAR, SUFFIX, seed=7, device=dev)
+    warm_layers, key = workload.scan_layers(sess, suffix, CHUNK)
+    warm_graph = esc.graph_capture(ctx, sess.set, 16384, warm_layers, stream)
+
+    def med_ms(fn, n=15, warm=2):
+        for _ in range(warm):
+            fn()
+        pairs = []
+        for _ in range(n):
+            flush_l2()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn()
+            b.record(stream)
+            pairs.append((a, b))
+        stream.synchronize()
+        t = sorted(_ev_ms(pairs))
+        return t[len(t) // 2], t
+
+    table = {}
+    for P in (2048, 4096, 8192, 16384):
+        T = P + SUFFIX
+        full = workload.SuffixInputs(N_LINEAR, T, seed=8, device=dev, distinct=False)
+        cold_layers, _ = workload.scan_layers(sess, full, CHUNK, cold=True)
+        cold_graph = esc.graph_capture(ctx, None, 0, cold_layers, stream)
+        cold_ms, _ = med_ms(lambda: cold_graph.launch(stream), n=15 if P <= 8192 else 7)
+        # warm: capsule at P (content: the session's current bytes), restore + 64-token suffix
+        slab = sess.new_slab(P)
+        sess.set.set_position(P)
+        cap = esc.snapshot(sess.set, P, CHUNK, slab, stream=stream)
+        warm_graph.set_capsule(cap, stream)
+        warm_ms, _ = med_ms(lambda: warm_graph.launch(stream))
+        restore_ms, _ = med_ms(lambda: esc.restore(sess.set, cap, stream=stream))
+        pay = cap.info().payload_bytes
+        table[str(P)] = {"cold_ms": cold_ms, "warm_ms": warm_ms, "speedup": cold_ms / warm_ms,
+                         "restore_us": restore_ms * 1e3, "restore_GBps": 2 * pay / (restore_ms * 1e-3) / 1e9,
+                         "capsule_MiB": pay / 2**20}
+        if P == 16384:
+            # one layer's cold scan alone: tokens/s and the HBM roofline of the scan kernel
+            q, k, v, g = full.dev[0]
+            one_ms, _ = med_ms(lambda: esc.linattn_scan(ctx, key, q, k, v, g, None, sess.states[0], full.out[0], T, T,
+                                                        CHUNK, stream=stream), n=7)
+            alg = T * workload.H * ALG_BYTES_PER_TOKEN_HEAD + 2 * workload.H * 128 * 128 * 4
+            gbs = alg / (one_ms * 1e-3) / 1e9
+            flops = T * workload.H * (2 * CHUNK * (128 + 128) + 4 * 128 * 128)
+            res["scan"] = {"tokens": T, "layers": 1, "ms": one_ms, "tokens_per_s": T / (one_ms * 1e-3),
+                           "tokens_per_s_18_layer_cold_graph": T / (cold_ms * 1e-3), "alg_TFLOPs": flops / (one_ms * 1e-3) / 1e12}
+            res["roofline_scan"] = {"kernel": "esc_scan_kernel<128,64,float> (B1 H16 d128 T=16448 chunk 64)", "bound": "hbm",
+                                    "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": gbs / pk["hbm_gbs"],
+                                    "peak_source": pk["source"], "traffic": None, "us_per_launch": one_ms * 1e3,
+                                    "alg_bytes_per_launch": alg}
+        cold_graph.destroy()
+        cap.destroy()
+        del full, slab
+        torch.cuda.empty_cache()
+    res["warm_vs_cold"] = {"note": "cold = 18 layers x scan(T=P+64) in one graph; warm = one graph [restore(P) + 18 x scan(64)]; "
+                                   "median of 15 (7 at 16k), L2 flushed; the scan only — the paper's TTFT includes the whole model",
+                           "by_prefix": table}
+    warm_graph.destroy()
+    return res
+
+
+if __name__ == "__main__":
+    _a = parse_args()
+    if _a.impl == "reference":
+        run_reference(_a)
+    else:
+        run_esc(_a)

@@ -54,6 +54,12 @@ class LiveSet:
                 self.host[i] = np.full(s.capacity_bytes, pattern, np.uint8)
             d.copy_(torch.from_numpy(self.host[i]))
 
+    def set_row(self, i, arr: np.ndarray):
+        """Overwrite the head of row i (device + host twin) with the bytes of `arr`."""
+        b = np.ascontiguousarray(arr).view(np.uint8).reshape(-1)
+        self.host[i][: b.size] = b
+        self.dev[i][: b.size].copy_(torch.from_numpy(b))
+
     def assert_equals_host(self):
         torch.cuda.synchronize()
         for d, h, s in zip(self.dev, self.host, self.specs):

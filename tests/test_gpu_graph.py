@@ -1,0 +1,122 @@
+"""-m gpu tests of the captured replay plan: restore + 18-layer suffix scan as ONE CUDA graph
+(BASELINE config 1), capsule swapped between replays without recapture."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_20537_b200 import synth
+from gpu_util import DEV, TOL_O, TOL_S, LiveSet, bits_equal, err_o, err_s, esc_mod, scan_dev_inputs
+
+pytestmark = pytest.mark.gpu
+
+B, H, DK, DV, CHUNK, SUFFIX = 1, 16, 128, 128, 64, 64
+
+
+@pytest.fixture(scope="module")
+def esc():
+    return esc_mod()
+
+
+@pytest.fixture(scope="module")
+def ctx(esc):
+    c = esc.Ctx(0)
+    yield c
+    c.close()
+
+
+def _hybrid_live(esc, ctx, t_max, seed):
+    specs = synth.hybrid_layout(t_max)
+    live = LiveSet(esc, ctx, specs, (20, seed))
+    lin = [i for i, s in enumerate(specs) if ".lin." in s.name]
+    for n, i in enumerate(lin):   # fold states must be finite floats, not random bytes
+        live.set_row(i, synth.scan_state(B, H, DK, DV, seed_ids=(20, seed, n), scale=0.3))
+    return live, lin
+
+
+def test_restore_plus_suffix_scan_graph(esc, ctx):
+    P = 2048
+    live, lin = _hybrid_live(esc, ctx, P + SUFFIX, 0)
+    states = [live.dev[i].view(torch.float32).view(B, H, DK, DV) for i in lin]
+    key = esc.shape_key_make(B, H, DK, DV, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
+    ins = [synth.scan_inputs(B, SUFFIX, H, DK, DV, seed_ids=(21, n)) for n in range(len(lin))]
+    dev_ins = [scan_dev_inputs(si) for si in ins]
+    outs = [torch.zeros((B, SUFFIX, H, DV), dtype=torch.float32, device=DEV) for _ in lin]
+
+    # two capsules with different contents (A: the initial live set; B: another prefill's bytes)
+    slab_a = torch.empty(live.set.capsule_bytes(P)[0], dtype=torch.uint8, device=DEV)
+    cap_a = esc.snapshot(live.set, P, CHUNK, slab_a)
+    s0_a = [s.clone() for s in states]
+    live.fill(22, 0)
+    for n, i in enumerate(lin):
+        live.set_row(i, synth.scan_state(B, H, DK, DV, seed_ids=(22, n), scale=0.3))
+    slab_b = torch.empty_like(slab_a)
+    cap_b = esc.snapshot(live.set, P, CHUNK, slab_b)
+    torch.cuda.synchronize()
+
+    def by_verbs(cap):
+        esc.restore(live.set, cap)
+        for n in range(len(lin)):
+            q, k, v, g = dev_ins[n]
+            esc.linattn_scan(ctx, key, q, k, v, g, states[n], states[n], outs[n], SUFFIX, SUFFIX, CHUNK)
+        torch.cuda.synchronize()
+        return [o.clone() for o in outs], [d.clone() for d in live.dev]
+
+    exp_a = by_verbs(cap_a)
+    exp_b = by_verbs(cap_b)
+    assert not bits_equal(exp_a[0][0], exp_b[0][0])
+
+    stream = torch.cuda.Stream()
+    layers = [esc.scan_args(key, *dev_ins[n], states[n], states[n], outs[n], SUFFIX, SUFFIX, CHUNK)
+              for n in range(len(lin))]
+    graph = esc.graph_capture(ctx, live.set, P, layers, stream)
+    with pytest.raises(esc.EscError):          # no capsule bound yet
+        graph.launch(stream)
+    for cap, (exp_o, exp_live) in ((cap_a, exp_a), (cap_b, exp_b), (cap_a, exp_a)):
+        live.fill(23, 0, pattern=0xFF)         # dirty every live buffer (NaN patterns)
+        for o in outs:
+            o.fill_(float("nan"))
+        torch.cuda.synchronize()
+        graph.set_capsule(cap, stream)         # swap the capsule: no recapture
+        graph.launch(stream)
+        stream.synchronize()
+        for o, e in zip(outs, exp_o):
+            assert bits_equal(o, e)
+        # live buffers: fold states advanced by the suffix, KV valid ranges restored; beyond-valid stays dirty
+        for i, (d, e) in enumerate(zip(live.dev, exp_live)):
+            sv = live.specs[i].fixed_bytes + P * live.specs[i].bytes_per_token
+            assert torch.equal(d[:sv], e[:sv]), live.specs[i].name
+            assert bool((d[sv:] == 0xFF).all())
+        assert live.set.position == P
+
+    # the graph's result against the oracle for one layer (state_in = capsule A's fold state)
+    q, k, v, g = ins[3].as_f32()
+    o_ref, s_ref = oracle.linattn_recurrence(q, k, v, g, s0_a[3].cpu().numpy().astype(np.float64))
+    assert err_o(outs[3].cpu().numpy(), o_ref) <= TOL_O
+    assert err_s(states[3].cpu().numpy(), s_ref) <= TOL_S
+    graph.destroy()
+
+
+def test_cold_plan_graph_matches_direct_calls(esc, ctx):
+    # a plan without a restore node: n layers of cold scans in one launch
+    T, n_layers = 512, 3
+    key = esc.shape_key_make(B, H, DK, DV, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
+    dev_ins = [scan_dev_inputs(synth.scan_inputs(B, T, H, DK, DV, seed_ids=(24, n))) for n in range(n_layers)]
+    st = [torch.empty((B, H, DK, DV), dtype=torch.float32, device=DEV) for _ in range(n_layers)]
+    outs = [torch.empty((B, T, H, DV), dtype=torch.float32, device=DEV) for _ in range(n_layers)]
+    for n in range(n_layers):
+        esc.linattn_scan(ctx, key, *dev_ins[n], None, st[n], outs[n], T, T, CHUNK)
+    torch.cuda.synchronize()
+    exp = [(o.clone(), s.clone()) for o, s in zip(outs, st)]
+    stream = torch.cuda.Stream()
+    graph = esc.graph_capture(ctx, None, 0, [esc.scan_args(key, *dev_ins[n], None, st[n], outs[n], T, T, CHUNK)
+                                             for n in range(n_layers)], stream)
+    for o, s in zip(outs, st):
+        o.fill_(float("nan"))
+        s.fill_(float("nan"))
+    torch.cuda.synchronize()
+    graph.launch(stream)
+    stream.synchronize()
+    for (eo, es_), o, s in zip(exp, outs, st):
+        assert bits_equal(o, eo) and bits_equal(s, es_)
+    graph.destroy()

@@ -1,0 +1,188 @@
+"""-m gpu parity tests of esc_linattn_scan through the C ABI against the fp64 sequential oracle.
+
+Bars (BASELINE.json north_star, metric readings #7/#8 of DESIGN.md):
+  o: ||o_gpu - o_ref||_inf / ||o_ref||_inf <= 2e-3 ;  S_T: relative Frobenius <= 1e-3 ;
+  chunk-aligned restore + continue == cold run, bit for bit;
+  bf16-o variant == RNE-bf16 of the fp32-o kernel's result, bit for bit."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_20537_b200 import synth
+from gpu_util import DEV, TOL_O, TOL_S, bits_equal, err_o, err_s, esc_mod, scan_dev_inputs, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def esc():
+    return esc_mod()
+
+
+@pytest.fixture(scope="module")
+def ctx(esc):
+    c = esc.Ctx(0)
+    yield c
+    c.close()
+
+
+def run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=None, t0=0, n=None, out_bf16=False, t_stride=None):
+    """Scan tokens [t0, t0+n) of device inputs laid out [B, t_stride, H, d]; returns (o[B,n,H,dv], S)."""
+    q, k, v, g = dev_in
+    t_stride = t_stride or q.shape[1]
+    n = T - t0 if n is None else n
+    key = esc.shape_key_make(B, H, dk, dv, esc.DTYPE_BF16, esc.DTYPE_BF16 if out_bf16 else esc.DTYPE_F32, chunk)
+    assert key
+    o = torch.full((B, t_stride, H, dv), float("nan"), dtype=torch.bfloat16 if out_bf16 else torch.float32, device=DEV)
+    s_out = torch.full((B, H, dk, dv), float("nan"), dtype=torch.float32, device=DEV)
+    esc.linattn_scan(ctx, key, q[:, t0:], k[:, t0:], v[:, t0:], g[:, t0:], s0, s_out, o[:, t0:], n, t_stride, chunk)
+    torch.cuda.synchronize()
+    return o[:, t0:t0 + n], s_out, o
+
+
+SHAPES = [
+    # B, H, dk, dv, T, chunk, gate
+    (1, 2, 64, 64, 256, 64, "fast"),        # BASELINE config 0
+    (2, 3, 128, 128, 300, 64, "fast"),      # several tiles + ragged tail
+    (1, 2, 64, 128, 130, 128, "fast"),
+    (1, 4, 128, 64, 257, 128, "fast"),
+    (1, 16, 128, 128, 512, 64, "fast"),     # config-1/2 head shape
+    (1, 2, 128, 128, 1024, 64, "slow"),     # slow decay: the carried state matters for many chunks
+    (1, 2, 128, 128, 640, 128, "slow"),
+    (1, 2, 64, 64, 256, 64, "one"),         # g == 1: plain linear attention
+    (1, 1, 128, 128, 1, 64, "fast"),        # T = 1
+    (1, 1, 128, 128, 63, 64, "fast"),       # T < chunk
+]
+
+
+@pytest.mark.parametrize("B,H,dk,dv,T,chunk,gate", SHAPES)
+@pytest.mark.parametrize("with_s0", [False, True])
+def test_scan_vs_oracle(esc, ctx, B, H, dk, dv, T, chunk, gate, with_s0):
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(10, T, dk, dv), gate=gate)
+    s0_np = synth.scan_state(B, H, dk, dv, seed_ids=(T,), scale=0.5) if with_s0 else None
+    o_ref, s_ref = oracle.linattn_recurrence(*si.as_f32(), None if s0_np is None else s0_np.astype(np.float64))
+    dev_in = scan_dev_inputs(si)
+    o, s, o_full = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, None if s0_np is None else to_dev(s0_np))
+    assert not torch.isnan(o).any() and not torch.isnan(s).any()
+    eo, es = err_o(o.cpu().numpy(), o_ref), err_s(s.cpu().numpy(), s_ref)
+    assert eo <= TOL_O, "o error %.3e" % eo
+    assert es <= TOL_S, "S error %.3e" % es
+    # bf16-o variant: RNE of the fp32 kernel's result, state identical
+    o16, s16, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, None if s0_np is None else to_dev(s0_np),
+                           out_bf16=True)
+    assert bits_equal(o16, o.to(torch.bfloat16)) and bits_equal(s16, s)
+
+
+def test_empty_T_copies_state(esc, ctx):
+    B, H, dk, dv = 1, 2, 64, 64
+    si = synth.scan_inputs(B, 4, H, dk, dv, seed_ids=(11,))
+    s0 = to_dev(synth.scan_state(B, H, dk, dv, seed_ids=(11,)))
+    _, s, _ = run_scan(esc, ctx, scan_dev_inputs(si), B, 0, H, dk, dv, 64, s0, n=0)
+    assert bits_equal(s, s0)
+    _, s, _ = run_scan(esc, ctx, scan_dev_inputs(si), B, 0, H, dk, dv, 64, None, n=0)
+    assert bool((s == 0).all())
+
+
+def test_batch_stride_and_untouched_tail(esc, ctx):
+    # only tokens [0,T) of each batch row are read / written; t_stride > T
+    B, H, dk, dv, Tbuf, T = 2, 2, 64, 64, 200, 150
+    si = synth.scan_inputs(B, Tbuf, H, dk, dv, seed_ids=(12,))
+    o_ref, s_ref = oracle.linattn_recurrence(*si.as_f32(), T=T)
+    o, s, o_full = run_scan(esc, ctx, scan_dev_inputs(si), B, T, H, dk, dv, 64, n=T)
+    assert err_o(o.cpu().numpy(), o_ref) <= TOL_O and err_s(s.cpu().numpy(), s_ref) <= TOL_S
+    assert torch.isnan(o_full[:, T:]).all(), "tokens beyond T were written"
+
+
+@pytest.mark.parametrize("B,H,dk,dv,T,chunk,P", [
+    (1, 2, 64, 64, 256, 64, 128),          # config 0: snapshot at t=128, restore, continue 128
+    (2, 4, 128, 128, 448, 64, 192),
+    (1, 4, 128, 128, 640, 128, 384),
+])
+def test_aligned_restore_continue_is_bit_identical_to_cold(esc, ctx, B, H, dk, dv, T, chunk, P):
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(13, T, P))
+    dev_in = scan_dev_inputs(si)
+    o_cold, s_cold, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk)
+    # prefill to P in a LIVE state buffer registered as a capsule row, snapshot, dirty, restore, continue
+    key = esc.shape_key_make(B, H, dk, dv, esc.DTYPE_BF16, esc.DTYPE_F32, chunk)
+    state = torch.zeros((B, H, dk, dv), dtype=torch.float32, device=DEV)
+    nbytes = state.numel() * 4
+    live = esc.bufset_create(ctx, [("L00.lin.state", state, nbytes, nbytes, 0, 1, 0)])
+    q, k, v, g = dev_in
+    o = torch.zeros((B, T, H, dv), dtype=torch.float32, device=DEV)
+    esc.linattn_scan(ctx, key, q, k, v, g, None, state, o, P, T, chunk)
+    assert esc.align_boundary(P, chunk) == P
+    slab = torch.empty(live.capsule_bytes(P)[0], dtype=torch.uint8, device=DEV)
+    cap = esc.snapshot(live, P, chunk, slab)
+    state.fill_(float("nan"))                       # dirty the live fold state
+    o[:, P:].fill_(float("nan"))
+    esc.restore(live, cap)
+    esc.linattn_scan(ctx, key, q[:, P:], k[:, P:], v[:, P:], g[:, P:], state, state, o[:, P:], T - P, T, chunk)
+    torch.cuda.synchronize()
+    assert bits_equal(o, o_cold), "restore+continue differs from the cold run"
+    assert bits_equal(state, s_cold)
+    # determinism: the cold run twice gives the same bits
+    o2, s2, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk)
+    assert bits_equal(o2, o_cold) and bits_equal(s2, s_cold)
+
+
+def test_misaligned_restore_is_within_tolerance(esc, ctx):
+    # a boundary off the chunk grid introduces a chunk split the cold run never had:
+    # tolerance-only against the oracle
+    B, H, dk, dv, T, chunk, P = 1, 4, 128, 128, 512, 64, 256 + 37
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(14,), gate="slow")
+    o_ref, s_ref = oracle.linattn_recurrence(*si.as_f32())
+    dev_in = scan_dev_inputs(si)
+    o_a, s_p, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, n=P)
+    o_b, s_t, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=s_p, t0=P)
+    o = torch.cat([o_a, o_b], dim=1)
+    assert err_o(o.cpu().numpy(), o_ref) <= TOL_O and err_s(s_t.cpu().numpy(), s_ref) <= TOL_S
+
+
+def test_kv_only_restore_diverges(esc, ctx):
+    # Table 8: dropping or staling the recurrent fold must be visible.  With the configured
+    # gate the state is forgotten in ~10 tokens, so the check looks at the first suffix tokens.
+    B, H, dk, dv, T, chunk, P = 1, 4, 128, 128, 256, 64, 128
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(15,))
+    o_ref, _ = oracle.linattn_recurrence(*si.as_f32())
+    dev_in = scan_dev_inputs(si)
+    _, s_p, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, n=P)
+    o_good, _, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=s_p, t0=P)
+    o_drop, _, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=None, t0=P)            # fold dropped
+    _, s_stale, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, n=P - 64)
+    o_stale, _, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=s_stale, t0=P)        # stale fold
+    head = slice(0, 10)
+    ref = o_ref[:, P:][:, head]
+    assert err_o(o_good[:, head].cpu().numpy(), ref) <= TOL_O
+    assert err_o(o_drop[:, head].cpu().numpy(), ref) > 10 * TOL_O
+    assert err_o(o_stale[:, head].cpu().numpy(), ref) > 10 * TOL_O
+
+
+def test_scan_argument_errors(esc, ctx):
+    key = esc.shape_key_make(1, 2, 64, 64, esc.DTYPE_BF16, esc.DTYPE_F32, 64)
+    t = torch.zeros(4096, dtype=torch.float32, device=DEV)
+    with pytest.raises(esc.EscError) as e:      # chunk differs from the key's
+        esc.linattn_scan(ctx, key, t, t, t, t, None, t, t, 1, 1, 128)
+    assert e.value.code == esc.ERR_MISMATCH
+    with pytest.raises(esc.EscError) as e:      # misaligned q
+        esc.linattn_scan(ctx, key, t.data_ptr() + 2, t, t, t, None, t, t, 1, 1, 64)
+    assert e.value.code == esc.ERR_UNALIGNED
+    with pytest.raises(esc.EscError) as e:      # t_stride < T
+        esc.linattn_scan(ctx, key, t, t, t, t, None, t, t, 8, 4, 64)
+    assert e.value.code == esc.ERR_INVALID
+    with pytest.raises(esc.EscError) as e:      # not a key
+        esc.linattn_scan(ctx, 12345, t, t, t, t, None, t, t, 1, 1, 64)
+    assert e.value.code == esc.ERR_INVALID
+
+
+def test_full_size_config2_sampled(esc, ctx):
+    # BASELINE config 2's cold scan at full size (B1 H16 d128, T = 16384 + 64, chunk 64) in the launch
+    # configuration bench.py times; the oracle checks a seeded sample of heads over the whole sequence.
+    B, H, dk, dv, T, chunk = 1, 16, 128, 128, 16384 + 64, 64
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(16,))
+    o, s, _ = run_scan(esc, ctx, scan_dev_inputs(si), B, T, H, dk, dv, chunk)
+    heads = [0, 7, 15]
+    q, k, v, g = si.as_f32()
+    o_ref, s_ref = oracle.linattn_recurrence(q[:, :, heads], k[:, :, heads], v[:, :, heads], g[:, :, heads])
+    assert err_o(o[:, :, heads].cpu().numpy(), o_ref) <= TOL_O
+    assert err_s(s[:, heads].cpu().numpy(), s_ref) <= TOL_S
