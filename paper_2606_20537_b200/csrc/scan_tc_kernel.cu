@@ -1,0 +1,579 @@
+// Chunked gated linear-attention scan, sm_100a tensor-core path (include/esc.h: esc_linattn_scan).
+//
+// Definition (BASELINE.json north_star; "a fold over the entire prefix", folded "per
+// chunk" PAPER.md:169):   S_t = g_t S_{t-1} + k_t^T v_t ,  o_t = q_t S_t.
+// Chunk algebra (exact-arithmetic equivalent; every exponent <= 0), with b_i = sum_{r<=i} log2 g_r:
+//     P      = Q K^T                                  (C x C)        tcgen05.mma  M=C  N=C  K=d_k
+//     A_ij   = P_ij 2^(b_i - b_j) [j <= i]            fp32 ALU + MUFU, split into bf16 hi + lo
+//     O1     = Q S_prev                               (C x 16)       tcgen05.mma  (S_prev hi + lo)
+//     O2     = A V                                    (C x 16)       tcgen05.mma  (A hi + lo)
+//     o_i    = 2^(b_i) O1_i + O2_i                    fp32 epilogue
+//     U      = K^T V~ ,  V~_j = 2^(b_C - b_j) v_j     (d_k x 16)     tcgen05.mma  (V~ hi + lo)
+//     S_next = 2^(b_C) S_prev + U                     fp32 FMA in registers (the carry chain)
+//
+// One CTA owns (b, h, 16 columns of d_v) — the columns of S are independent — and walks the chunks
+// in order.  Only the last line is a true dependency between chunks: P, A, O2, U of later chunks do
+// not depend on S, so the kernel is a software pipeline of specialised warps
+//   warp 0      TMA producer: Q / K / V chunk tiles -> 128B/32B-swizzled shared memory, NS-stage ring
+//   warp 1      MMA issuer: one thread issues every tcgen05.mma; accumulators live in TMEM
+//   warp 2      gate warp: log2 g, segmented warp-shuffle prefix sums for 256 tokens at a time
+//   warps 3-6   score warps: P (TMEM) -> A hi/lo (smem, UMMA K-major interleaved), V -> V~ hi/lo
+//   warps 7-10  state warps: U (TMEM) -> carry S in registers -> S hi/lo operand; O1,O2 -> o (global)
+// synchronised only by mbarriers (TMA complete_tx, tcgen05.commit, warp arrivals).
+//
+// Bit-identity: the carry is a pure function of (S_prev bits, chunk inputs); there
+// is no T-dependent tiling, no atomics, no split-K; the MMA issue order inside a chunk is fixed.
+// Precision: raw Q, K, V are bf16 inputs; A, V~, S_prev are two-term bf16 splits.
+#include <cuda.h>
+#include <cuda_bf16.h>
+
+#include "esc_internal.h"
+#include "sm100_ptx.cuh"
+
+namespace esc {
+
+using namespace ptx;
+typedef __nv_bfloat16 bf16;
+
+constexpr int kTcThreads = 352;   // 11 warps
+constexpr int kTcDVT = 16;        // d_v columns per CTA
+constexpr int kGateBatch = 256;   // tokens per gate-warp batch
+
+template <int DK, int C>
+struct TcCfg {
+    static constexpr int NS = (C == 64) ? 3 : 2;          // input stages
+    static constexpr int NB = (C == 64) ? 2 : 1;          // P / A / V~ buffers
+    static constexpr int NH = DK / 64;                    // 64-column halves of a Q / K tile
+    static constexpr int CPB = kGateBatch / C;            // chunks per gate batch
+    static constexpr uint32_t half_bytes = C * 128;       // one [C x 64] bf16 half tile
+    static constexpr uint32_t q_bytes = NH * half_bytes;
+    static constexpr uint32_t v_bytes = C * 32;           // [C x 16] bf16
+    static constexpr uint32_t stage_bytes = 2 * q_bytes + v_bytes;   // multiple of 1024
+    static constexpr uint32_t a_bytes = C * C * 2;        // one A term
+    static constexpr uint32_t vt_bytes = C * kTcDVT * 2;  // one V~ term
+    static constexpr uint32_t s_bytes = DK * kTcDVT * 2;  // one S term
+    // offsets from the 1024-aligned base
+    static constexpr uint32_t stage_off = 0;
+    static constexpr uint32_t a_off = stage_off + NS * stage_bytes;             // [NB][hi,lo]
+    static constexpr uint32_t vt_off = a_off + NB * 2 * a_bytes;                // [NB][hi,lo]
+    static constexpr uint32_t s_off = vt_off + NB * 2 * vt_bytes;               // [hi,lo]
+    static constexpr uint32_t gate_off = s_off + 2 * s_bytes;                   // [2][b2[256], eb[256]] fp32
+    static constexpr uint32_t bar_off = gate_off + 2 * 2 * kGateBatch * 4;
+    static constexpr uint32_t n_bars = 2 * NS + 4 * NB + 2 + 2 + 2 * 2 + 2 * 2 + 2 * 2;
+    static constexpr uint32_t total = bar_off + 64 * 8 + 16 + 1024;             // + alignment slack
+    static constexpr uint32_t tmem_cols = 256;
+    static constexpr uint32_t tm_p = 0;                    // [NB] x C columns
+    static constexpr uint32_t tm_u = NB * C;               // [2] x 16
+    static constexpr uint32_t tm_o1 = tm_u + 32;           // [2] x 16
+    static constexpr uint32_t tm_o2 = tm_o1 + 32;          // [2] x 16
+    static_assert(tm_o2 + 32 <= tmem_cols, "TMEM budget");
+    static_assert(stage_bytes % 1024 == 0, "stages must keep 1024-byte alignment (128B swizzle)");
+    static_assert(n_bars <= 64, "barrier area");
+};
+
+struct TcBars {   // indices into the mbarrier array
+    int full, empty, p_full, p_empty, a_full, a_empty, s_full, s_empty, o_full, o_empty, u_full, u_empty, g_full, g_empty;
+};
+template <int DK, int C>
+__device__ __forceinline__ constexpr TcBars tc_bars() {
+    using L = TcCfg<DK, C>;
+    TcBars b{};
+    int i = 0;
+    b.full = i; i += L::NS;
+    b.empty = i; i += L::NS;
+    b.p_full = i; i += L::NB;
+    b.p_empty = i; i += L::NB;
+    b.a_full = i; i += L::NB;
+    b.a_empty = i; i += L::NB;
+    b.s_full = i; i += 1;
+    b.s_empty = i; i += 1;
+    b.o_full = i; i += 2;
+    b.o_empty = i; i += 2;
+    b.u_full = i; i += 2;
+    b.u_empty = i; i += 2;
+    b.g_full = i; i += 2;
+    b.g_empty = i; i += 2;
+    return b;
+}
+
+__device__ __forceinline__ uint32_t pack_bf16(float lo_elem, float hi_elem) {   // element 0 in the low half
+    __nv_bfloat162 p = __floats2bfloat162_rn(lo_elem, hi_elem);
+    return *reinterpret_cast<uint32_t*>(&p);
+}
+// two-term split of a pair: returns packed hi terms, writes packed lo terms
+__device__ __forceinline__ uint32_t split2(float x0, float x1, uint32_t& lo) {
+    const bf16 h0 = __float2bfloat16_rn(x0), h1 = __float2bfloat16_rn(x1);
+    lo = pack_bf16(x0 - __bfloat162float(h0), x1 - __bfloat162float(h1));
+    __nv_bfloat162 p;
+    p.x = h0;
+    p.y = h1;
+    return *reinterpret_cast<uint32_t*>(&p);
+}
+__device__ __forceinline__ float ex2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+template <typename OutT>
+__device__ __forceinline__ void store_o2(OutT* p, float x0, float x1);
+template <>
+__device__ __forceinline__ void store_o2<float>(float* p, float x0, float x1) {
+    *reinterpret_cast<float2*>(p) = make_float2(x0, x1);
+}
+template <>
+__device__ __forceinline__ void store_o2<bf16>(bf16* p, float x0, float x1) {
+    *reinterpret_cast<uint32_t*>(p) = pack_bf16(x0, x1);
+}
+
+template <int DK, int C, typename OutT>
+__global__ void __launch_bounds__(kTcThreads, 1)
+esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tk,
+                   const __grid_constant__ CUtensorMap tv, const float* __restrict__ g, const float* state_in,
+                   float* state_out, OutT* __restrict__ o, uint32_t H, uint32_t DV, uint64_t T, uint64_t t_stride) {
+    using L = TcCfg<DK, C>;
+    constexpr TcBars BI = tc_bars<DK, C>();
+    constexpr int NS = L::NS, NB = L::NB, CPB = L::CPB;
+    constexpr uint32_t SBO_A = (C / 8) * 128, SBO_V = (C / 8) * 128, SBO_S = (DK / 8) * 128;
+
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    const uint32_t sm_a = smem_u32(sm);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sm + L::bar_off);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sm + L::bar_off + 64 * 8);
+    float* gate = reinterpret_cast<float*>(sm + L::gate_off);   // [2][2][256]: b2 then eb per slot
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t bh = blockIdx.y, b = bh / H, h = bh % H, dv0 = blockIdx.x * kTcDVT;
+    const uint32_t n_chunks = (uint32_t)((T + C - 1) / C);
+    const int q = warp & 3;   // TMEM lane quadrant this warp may access
+
+    // ---- one-time setup ----------------------------------------------------------------------------
+    if (warp == 0 && lane == 0) {
+        for (int i = 0; i < NS; ++i) { mbar_init(&bars[BI.full + i], 1); mbar_init(&bars[BI.empty + i], 5); }
+        for (int i = 0; i < NB; ++i) {
+            mbar_init(&bars[BI.p_full + i], 1); mbar_init(&bars[BI.p_empty + i], 4);
+            mbar_init(&bars[BI.a_full + i], 4); mbar_init(&bars[BI.a_empty + i], 1);
+        }
+        mbar_init(&bars[BI.s_full], 4); mbar_init(&bars[BI.s_empty], 1);
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(&bars[BI.o_full + i], 1); mbar_init(&bars[BI.o_empty + i], 4);
+            mbar_init(&bars[BI.u_full + i], 1); mbar_init(&bars[BI.u_empty + i], 4);
+            mbar_init(&bars[BI.g_full + i], 1); mbar_init(&bars[BI.g_empty + i], 8);
+        }
+        fence_mbar_init();
+        tma_prefetch_desc(&tq); tma_prefetch_desc(&tk); tma_prefetch_desc(&tv);
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, L::tmem_cols);
+    // A buffers: the strictly-upper 16x16 blocks are never written again and must read as zero
+    for (uint32_t i = threadIdx.x; i < NB * 2 * L::a_bytes / 16; i += kTcThreads)
+        reinterpret_cast<uint4*>(sm + L::a_off)[i] = make_uint4(0, 0, 0, 0);
+
+    // state warps own the carry: row `krow` of the [d_k x 16] slice per thread, fp32 registers
+    const bool st_warp = warp >= 7;
+    const bool st_active = st_warp && (DK == 128 || lane < 16);
+    const uint32_t krow = (DK == 128) ? 32 * q + lane : 16 * q + (lane & 15);
+    float S[16];
+    auto write_s_operand = [&]() {   // S hi/lo as UMMA B operand, MN-major interleaved: (n,k) -> (n/8)*SBO + (k/8)*128 + (k%8)*16
+        if (st_active) {
+#pragma unroll
+            for (int nb = 0; nb < 2; ++nb) {
+                uint4 hi, lo;
+                hi.x = split2(S[8 * nb + 0], S[8 * nb + 1], lo.x);
+                hi.y = split2(S[8 * nb + 2], S[8 * nb + 3], lo.y);
+                hi.z = split2(S[8 * nb + 4], S[8 * nb + 5], lo.z);
+                hi.w = split2(S[8 * nb + 6], S[8 * nb + 7], lo.w);
+                const uint32_t off = nb * SBO_S + (krow >> 3) * 128 + (krow & 7) * 16;
+                *reinterpret_cast<uint4*>(sm + L::s_off + off) = hi;
+                *reinterpret_cast<uint4*>(sm + L::s_off + L::s_bytes + off) = lo;
+            }
+        }
+    };
+    if (st_warp) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) S[j] = 0.f;
+        if (st_active && state_in) {
+            const float4* p = reinterpret_cast<const float4*>(state_in + ((size_t)bh * DK + krow) * DV + dv0);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float4 x = p[j];
+                S[4 * j] = x.x; S[4 * j + 1] = x.y; S[4 * j + 2] = x.z; S[4 * j + 3] = x.w;
+            }
+        }
+        write_s_operand();
+    }
+    fence_proxy_async_smem();
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
+    const uint32_t tb = *tmem_slot;
+    if (st_warp && lane == 0) mbar_arrive(&bars[BI.s_full]);   // version 0 of the S operand is in place
+
+    if (warp == 0) {
+        // ================= TMA producer =================
+        if (lane == 0) {
+            for (uint32_t c = 0; c < n_chunks; ++c) {
+                const uint32_t s = c % NS;
+                mbar_wait(&bars[BI.empty + s], ((c / NS) & 1) ^ 1);
+                uint8_t* st = sm + L::stage_off + s * L::stage_bytes;
+                uint64_t* full = &bars[BI.full + s];
+                mbar_arrive_expect_tx(full, L::stage_bytes);
+                const int t0 = (int)(c * C);
+#pragma unroll
+                for (int hh = 0; hh < L::NH; ++hh) {
+                    tma_load_4d(st + hh * L::half_bytes, &tq, full, hh * 64, (int)h, t0, (int)b);
+                    tma_load_4d(st + L::q_bytes + hh * L::half_bytes, &tk, full, hh * 64, (int)h, t0, (int)b);
+                }
+                tma_load_4d(st + 2 * L::q_bytes, &tv, full, (int)dv0, (int)h, t0, (int)b);
+            }
+        }
+    } else if (warp == 1) {
+        // ================= MMA issuer (one thread) =================
+        if (lane == 0) {
+            constexpr uint32_t idP = idesc_bf16(C, C, 0, 0);
+            constexpr uint32_t idO = idesc_bf16(C, kTcDVT, 0, 1);
+            constexpr uint32_t idU = idesc_bf16(DK, kTcDVT, 1, 1);
+            auto issue_P = [&](uint32_t c) {
+                const uint32_t s = c % NS, pb = c % NB;
+                mbar_wait(&bars[BI.full + s], (c / NS) & 1);
+                mbar_wait(&bars[BI.p_empty + pb], ((c / NB) & 1) ^ 1);
+                tc_fence_after_sync();
+                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes, ka = qa + L::q_bytes;
+#pragma unroll
+                for (int ks = 0; ks < DK / 16; ++ks) {
+                    const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
+                    mma_bf16_ss(tb + L::tm_p + pb * C, smem_desc(qa + off, 16, 1024, kSwz128),
+                                smem_desc(ka + off, 16, 1024, kSwz128), idP, ks > 0);
+                }
+                mma_commit(&bars[BI.p_full + pb]);
+            };
+            auto issue_O1 = [&](uint32_t c) {
+                const uint32_t s = c % NS, ob = c & 1;
+                mbar_wait(&bars[BI.s_full], c & 1);
+                mbar_wait(&bars[BI.o_empty + ob], ((c >> 1) & 1) ^ 1);
+                tc_fence_after_sync();
+                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes;
+#pragma unroll
+                for (int term = 0; term < 2; ++term) {
+#pragma unroll
+                    for (int ks = 0; ks < DK / 16; ++ks) {
+                        const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
+                        mma_bf16_ss(tb + L::tm_o1 + ob * 16, smem_desc(qa + off, 16, 1024, kSwz128),
+                                    smem_desc(sm_a + L::s_off + term * L::s_bytes + 2 * ks * 128, 128, SBO_S, kSwzNone), idO,
+                                    (term | ks) > 0);
+                    }
+                }
+                mma_commit(&bars[BI.s_empty]);
+            };
+            auto issue_UO2 = [&](uint32_t c) {
+                const uint32_t s = c % NS, pb = c % NB, ob = c & 1;
+                mbar_wait(&bars[BI.a_full + pb], (c / NB) & 1);
+                mbar_wait(&bars[BI.u_empty + ob], ((c >> 1) & 1) ^ 1);
+                tc_fence_after_sync();
+                const uint32_t ka = sm_a + L::stage_off + s * L::stage_bytes + L::q_bytes, va = ka + L::q_bytes;
+                const uint32_t vt = sm_a + L::vt_off + pb * 2 * L::vt_bytes, aa = sm_a + L::a_off + pb * 2 * L::a_bytes;
+#pragma unroll
+                for (int term = 0; term < 2; ++term) {   // U = K^T V~ : A operand = the K tile read MN-major
+#pragma unroll
+                    for (int ks = 0; ks < C / 16; ++ks)
+                        mma_bf16_ss(tb + L::tm_u + ob * 16, smem_desc(ka + 2 * ks * 1024, L::half_bytes, 1024, kSwz128),
+                                    smem_desc(vt + term * L::vt_bytes + 2 * ks * 128, 128, SBO_V, kSwzNone), idU, (term | ks) > 0);
+                }
+                mma_commit(&bars[BI.u_full + ob]);
+#pragma unroll
+                for (int term = 0; term < 2; ++term) {   // O2 = A V : B operand = the V tile read MN-major (32B swizzle)
+#pragma unroll
+                    for (int ks = 0; ks < C / 16; ++ks)
+                        mma_bf16_ss(tb + L::tm_o2 + ob * 16, smem_desc(aa + term * L::a_bytes + 2 * ks * 128, 128, SBO_A, kSwzNone),
+                                    smem_desc(va + 2 * ks * 256, 512, 256, kSwz32), idO, (term | ks) > 0);
+                }
+                mma_commit(&bars[BI.o_full + ob]);
+                mma_commit(&bars[BI.a_empty + pb]);
+                mma_commit(&bars[BI.empty + s]);
+            };
+            if (n_chunks) issue_P(0);
+            for (uint32_t c = 0; c < n_chunks; ++c) {
+                if (c + 1 < n_chunks) issue_P(c + 1);   // keeps the tensor pipe busy while the score warps build A(c)
+                issue_O1(c);
+                issue_UO2(c);
+            }
+        }
+    } else if (warp == 2) {
+        // ================= gate warp: b2_i = sum_{r<=i in chunk} log2 g_r, 256 tokens per batch =================
+        const uint32_t n_batches = (uint32_t)((T + kGateBatch - 1) / kGateBatch);
+        constexpr int GL = C / 8;   // lanes per chunk
+        float gv[8];
+        auto load_g = [&](uint32_t bt) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const uint64_t tt = (uint64_t)bt * kGateBatch + 8 * lane + u;
+                gv[u] = tt < T ? g[((size_t)b * t_stride + tt) * H + h] : 1.f;
+            }
+        };
+        if (n_batches) load_g(0);
+        for (uint32_t bt = 0; bt < n_batches; ++bt) {
+            float loc[8], run = 0.f;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                run += log2f(gv[u]);
+                loc[u] = run;
+            }
+            if (bt + 1 < n_batches) load_g(bt + 1);   // next batch's loads fly while this one is scanned
+            float incl = run;
+#pragma unroll
+            for (int d = 1; d < GL; d <<= 1) {
+                const float up = __shfl_up_sync(0xffffffffu, incl, d);
+                if ((lane % GL) >= d) incl += up;
+            }
+            const float prev = __shfl_up_sync(0xffffffffu, incl, 1);
+            const float excl = (lane % GL) ? prev : 0.f;
+            const uint32_t slot = bt & 1;
+            mbar_wait(&bars[BI.g_empty + slot], ((bt >> 1) & 1) ^ 1);
+            float* b2 = gate + slot * 2 * kGateBatch;
+            float* eb = b2 + kGateBatch;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const float x = excl + loc[u];
+                b2[8 * lane + u] = x;
+                eb[8 * lane + u] = ex2(x);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars[BI.g_full + slot]);
+        }
+    }
+    else if (warp < 7) {
+        // ================= score warps: A = P ⊙ 2^(b_i - b_j) (causal), V~ = V ⊙ 2^(b_C - b_j) =================
+        const int tid_wg = (warp - 3) * 32 + lane;
+        constexpr int NG = C / 64;                 // 16-row groups per warp (row r of an M=64 tile sits in lane 32(r/16)+r%16)
+        for (uint32_t c = 0; c < n_chunks; ++c) {
+            const uint32_t s = c % NS, pb = c % NB, bt = c / CPB, gslot = bt & 1;
+            mbar_wait(&bars[BI.g_full + gslot], (bt >> 1) & 1);
+            const float* b2 = gate + gslot * 2 * kGateBatch + (c % CPB) * C;
+            mbar_wait(&bars[BI.full + s], (c / NS) & 1);
+            mbar_wait(&bars[BI.a_empty + pb], ((c / NB) & 1) ^ 1);
+            {   // V~ hi/lo, UMMA B operand MN-major interleaved: (n,k=token) -> (n/8)*SBO_V + (k/8)*128 + (k%8)*16 + (n%8)*2
+                const uint8_t* vs = sm + L::stage_off + s * L::stage_bytes + 2 * L::q_bytes;
+                uint8_t* vt = sm + L::vt_off + pb * 2 * L::vt_bytes;
+                const float b_last = b2[C - 1];
+                for (int idx = tid_wg; idx < C * 2; idx += 128) {
+                    const int j = idx >> 1, half = idx & 1;
+                    const uint4 raw = *reinterpret_cast<const uint4*>(vs + j * 32 + ((half ^ ((j >> 2) & 1)) * 16));   // undo 32B swizzle
+                    const float sc = ex2(b_last - b2[j]);
+                    const uint32_t w[4] = {raw.x, raw.y, raw.z, raw.w};
+                    uint32_t hi[4], lo[4];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const float x0 = __uint_as_float(w[e] << 16) * sc, x1 = __uint_as_float(w[e] & 0xFFFF0000u) * sc;
+                        hi[e] = split2(x0, x1, lo[e]);
+                    }
+                    const uint32_t off = half * SBO_V + (j >> 3) * 128 + (j & 7) * 16;
+                    *reinterpret_cast<uint4*>(vt + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+                    *reinterpret_cast<uint4*>(vt + L::vt_bytes + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+                }
+            }
+            mbar_wait(&bars[BI.p_full + pb], (c / NB) & 1);
+            tc_fence_after_sync();
+            uint8_t* ah = sm + L::a_off + pb * 2 * L::a_bytes;
+#pragma unroll
+            for (int gi = 0; gi < NG; ++gi) {
+                const int rg = (C == 64) ? q : 2 * q + gi;             // 16-row group index
+                const uint32_t lane_base = (C == 64) ? 32 * q : 32 * q + 16 * gi;
+                uint32_t r[C / 16][8];
+#pragma unroll
+                for (int cb = 0; cb < C / 16; ++cb)
+                    if (cb <= rg) tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_p + pb * C + cb * 16), r[cb]);
+                tmem_ld_wait();
+                if (gi == NG - 1) {   // P(c) is in registers: the MMA thread may overwrite this TMEM buffer
+                    tc_fence_before_sync();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&bars[BI.p_empty + pb]);
+                }
+                const int ra = 16 * rg + (lane >> 2), rb = ra + 8;
+                const float ba = b2[ra], bb = b2[rb];
+#pragma unroll
+                for (int cb = 0; cb < C / 16; ++cb) {
+                    if (cb <= rg) {
+#pragma unroll
+                        for (int jb = 0; jb < 2; ++jb) {
+                            const int j0 = cb * 16 + jb * 8 + 2 * (lane & 3);
+                            const float2 bj = *reinterpret_cast<const float2*>(b2 + j0);
+                            float a0 = __uint_as_float(r[cb][4 * jb + 0]) * ex2(ba - bj.x);
+                            float a1 = __uint_as_float(r[cb][4 * jb + 1]) * ex2(ba - bj.y);
+                            float c0 = __uint_as_float(r[cb][4 * jb + 2]) * ex2(bb - bj.x);
+                            float c1 = __uint_as_float(r[cb][4 * jb + 3]) * ex2(bb - bj.y);
+                            if (cb == rg) {   // diagonal block: causal mask j <= i
+                                a0 = (j0 <= ra) ? a0 : 0.f;
+                                a1 = (j0 + 1 <= ra) ? a1 : 0.f;
+                                c0 = (j0 <= rb) ? c0 : 0.f;
+                                c1 = (j0 + 1 <= rb) ? c1 : 0.f;
+                            }
+                            uint32_t lo_a, lo_c;
+                            const uint32_t hi_a = split2(a0, a1, lo_a), hi_c = split2(c0, c1, lo_c);
+                            // UMMA A operand, K-major interleaved: (i,j) -> (i/8)*SBO_A + (j/8)*128 + (i%8)*16 + (j%8)*2
+                            const uint32_t oa = (ra >> 3) * SBO_A + (j0 >> 3) * 128 + (ra & 7) * 16 + (j0 & 7) * 2;
+                            const uint32_t oc = (rb >> 3) * SBO_A + (j0 >> 3) * 128 + (rb & 7) * 16 + (j0 & 7) * 2;
+                            *reinterpret_cast<uint32_t*>(ah + oa) = hi_a;
+                            *reinterpret_cast<uint32_t*>(ah + L::a_bytes + oa) = lo_a;
+                            *reinterpret_cast<uint32_t*>(ah + oc) = hi_c;
+                            *reinterpret_cast<uint32_t*>(ah + L::a_bytes + oc) = lo_c;
+                        }
+                    }
+                }
+            }
+            fence_proxy_async_smem();   // generic-proxy writes of A, V~ -> visible to tcgen05.mma's operand reads
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(&bars[BI.a_full + pb]);
+                mbar_arrive(&bars[BI.empty + s]);
+                if ((c % CPB) == CPB - 1 || c + 1 == n_chunks) mbar_arrive(&bars[BI.g_empty + gslot]);
+            }
+        }
+    } else {
+        // ================= state warps: carry S, emit o =================
+        constexpr int NG = C / 64;
+        for (uint32_t c = 0; c < n_chunks; ++c) {
+            const uint32_t ob = c & 1, bt = c / CPB, gslot = bt & 1;
+            mbar_wait(&bars[BI.g_full + gslot], (bt >> 1) & 1);
+            const float* eb = gate + gslot * 2 * kGateBatch + kGateBatch + (c % CPB) * C;
+            // ---- the carry: S <- 2^(b_C) S + U, fp32 FMA in registers ----
+            mbar_wait(&bars[BI.u_full + ob], (c >> 1) & 1);
+            tc_fence_after_sync();
+            uint32_t ur[16];
+            tmem_ld_32x32b_x16(tmem_addr(tb, 32 * q, L::tm_u + ob * 16), ur);
+            tmem_ld_wait();
+            tc_fence_before_sync();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars[BI.u_empty + ob]);
+            const float gam = eb[C - 1];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) S[j] = fmaf(gam, S[j], __uint_as_float(ur[j]));
+            if (c + 1 < n_chunks) {
+                mbar_wait(&bars[BI.s_empty], c & 1);   // O1(c) has finished reading the previous operand
+                write_s_operand();
+                fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bars[BI.s_full]);
+            }
+            // ---- epilogue: o_i = 2^(b_i) O1_i + O2_i ----
+            mbar_wait(&bars[BI.o_full + ob], (c >> 1) & 1);
+            tc_fence_after_sync();
+            const uint64_t t0 = (uint64_t)c * C;
+            const int n = (int)((T - t0) < (uint64_t)C ? (T - t0) : (uint64_t)C);
+#pragma unroll
+            for (int gi = 0; gi < NG; ++gi) {
+                const int rg = (C == 64) ? q : 2 * q + gi;
+                const uint32_t lane_base = (C == 64) ? 32 * q : 32 * q + 16 * gi;
+                uint32_t r1[8], r2[8];
+                tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_o1 + ob * 16), r1);
+                tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_o2 + ob * 16), r2);
+                tmem_ld_wait();
+                if (gi == NG - 1) {
+                    tc_fence_before_sync();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&bars[BI.o_empty + ob]);
+                }
+                const int ra = 16 * rg + (lane >> 2), rb = ra + 8;
+                const float ea = eb[ra], ebb = eb[rb];
+                OutT* oa = o + (((size_t)b * t_stride + t0 + ra) * H + h) * DV + dv0 + 2 * (lane & 3);
+                OutT* oc = o + (((size_t)b * t_stride + t0 + rb) * H + h) * DV + dv0 + 2 * (lane & 3);
+#pragma unroll
+                for (int jb = 0; jb < 2; ++jb) {
+                    if (ra < n)
+                        store_o2<OutT>(oa + jb * 8, fmaf(ea, __uint_as_float(r1[4 * jb + 0]), __uint_as_float(r2[4 * jb + 0])),
+                                       fmaf(ea, __uint_as_float(r1[4 * jb + 1]), __uint_as_float(r2[4 * jb + 1])));
+                    if (rb < n)
+                        store_o2<OutT>(oc + jb * 8, fmaf(ebb, __uint_as_float(r1[4 * jb + 2]), __uint_as_float(r2[4 * jb + 2])),
+                                       fmaf(ebb, __uint_as_float(r1[4 * jb + 3]), __uint_as_float(r2[4 * jb + 3])));
+                }
+            }
+            __syncwarp();
+            if (lane == 0 && ((c % CPB) == CPB - 1 || c + 1 == n_chunks)) mbar_arrive(&bars[BI.g_empty + gslot]);
+        }
+        if (st_active) {
+            float4* p = reinterpret_cast<float4*>(state_out + ((size_t)bh * DK + krow) * DV + dv0);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) p[j] = make_float4(S[4 * j], S[4 * j + 1], S[4 * j + 2], S[4 * j + 3]);
+        }
+    }
+
+    // ---- teardown: every tcgen05 op has completed (the state warps waited on the last commits) ----
+    tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tb, L::tmem_cols);
+}
+
+// ---- host ---------------------------------------------------------------------------------------
+typedef CUresult (*TmapEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static TmapEncodeFn tmap_encode_fn() {
+    static TmapEncodeFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+            qres != cudaDriverEntryPointSuccess)
+            p = nullptr;
+        return (TmapEncodeFn)p;
+    }();
+    return fn;
+}
+
+// 4-D map over a [B, t_stride, H, D] bf16 tensor whose first `T` tokens per batch row are valid:
+// dims (D, H, T, B), box (box_d, 1, C, 1).  Rows beyond T read as zero (the short last chunk).
+static int make_tmap(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, uint64_t T, uint64_t t_stride, uint32_t B,
+                     uint32_t box_d, uint32_t box_t, CUtensorMapSwizzle sw) {
+    TmapEncodeFn enc = tmap_encode_fn();
+    if (!enc) return ESC_ERR_CUDA;
+    cuuint64_t dims[4] = {D, H, T ? T : 1, B};
+    cuuint64_t strides[3] = {(cuuint64_t)D * 2, (cuuint64_t)H * D * 2, (cuuint64_t)t_stride * H * D * 2};
+    cuuint32_t box[4] = {box_d, 1, box_t, 1};
+    cuuint32_t es[4] = {1, 1, 1, 1};
+    if (B == 1) strides[2] = strides[1] * dims[2];   // unused dimension: any valid multiple of 16
+    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box, es,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? ESC_OK : ESC_ERR_CUDA;
+}
+
+template <int DK, int C, typename OutT>
+static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
+                       float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
+    using L = TcCfg<DK, C>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        ESC_CUDA(cudaFuncSetAttribute(esc_scan_tc_kernel<DK, C, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::total));
+        attr_set = true;
+    }
+    if (!state_out) return ESC_OK;   // prepare-only call (before a stream capture)
+    CUtensorMap tq, tk, tv;
+    const void* qq = T ? q : (const void*)state_out;   // T == 0: maps are never dereferenced, any valid address will do
+    const void* kk = T ? k : (const void*)state_out;
+    const void* vv = T ? v : (const void*)state_out;
+    int rc = make_tmap(&tq, qq, DK, s.H, T, t_stride ? t_stride : 1, s.B, 64, C, CU_TENSOR_MAP_SWIZZLE_128B);
+    if (rc == ESC_OK) rc = make_tmap(&tk, kk, DK, s.H, T, t_stride ? t_stride : 1, s.B, 64, C, CU_TENSOR_MAP_SWIZZLE_128B);
+    if (rc == ESC_OK) rc = make_tmap(&tv, vv, s.dv, s.H, T, t_stride ? t_stride : 1, s.B, kTcDVT, C, CU_TENSOR_MAP_SWIZZLE_32B);
+    if (rc != ESC_OK) return rc;
+    dim3 grid(s.dv / kTcDVT, s.B * s.H);
+    esc_scan_tc_kernel<DK, C, OutT><<<grid, kTcThreads, L::total, stream>>>(tq, tk, tv, g, state_in, state_out, (OutT*)o, s.H,
+                                                                             s.dv, T, t_stride);
+    ESC_CUDA(cudaGetLastError());
+    return ESC_OK;
+}
+
+template <int DK, int C>
+static int launch_tc_o(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
+                       float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
+    if (s.out_dtype == ESC_DTYPE_F32) return launch_tc_t<DK, C, float>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    return launch_tc_t<DK, C, bf16>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+}
+
+int launch_scan_tc(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
+                   float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
+    if (s.dk == 128 && s.chunk == 64) return launch_tc_o<128, 64>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 128 && s.chunk == 128) return launch_tc_o<128, 128>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 64 && s.chunk == 64) return launch_tc_o<64, 64>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 64 && s.chunk == 128) return launch_tc_o<64, 128>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    return ESC_ERR_UNSUPPORTED;
+}
+
+}  // namespace esc
