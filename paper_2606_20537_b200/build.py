@@ -16,7 +16,7 @@ TARGET = os.path.join(PKG, "libesc.so")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-DESC_BUILD",
+    "-Xcompiler", "-fPIC", "-DESC_BUILD",] + (["-DESC_TC_TRACE"] if os.environ.get("ESC_TC_TRACE") else []) + [
     "-I", os.path.join(ROOT, "include"), "-I", CSRC,
 ]
 

@@ -17,8 +17,8 @@
 //   warp 0      TMA producer: Q / K / V chunk tiles -> 128B/32B-swizzled shared memory, NS-stage ring
 //   warp 1      MMA issuer: one thread issues every tcgen05.mma; accumulators live in TMEM
 //   warp 2      gate warp: log2 g, segmented warp-shuffle prefix sums for 256 tokens at a time
-//   warps 3-6   score warps: P (TMEM) -> A hi/lo (smem, UMMA K-major interleaved), V -> V~ hi/lo
-//   warps 7-10  state warps: U (TMEM) -> carry S in registers -> S hi/lo operand; O1,O2 -> o (global)
+//   warps 4-11  score warps (2 groups): P (TMEM) -> A hi/lo (smem, UMMA K-major interleaved), V -> V~ hi/lo
+//   warps 12-15 state warps: U (TMEM) -> carry S in registers -> S hi/lo operand; O1,O2 -> o (global)
 // synchronised only by mbarriers (TMA complete_tx, tcgen05.commit, warp arrivals).
 //
 // Bit-identity: the carry is a pure function of (S_prev bits, chunk inputs); there
@@ -35,14 +35,23 @@ namespace esc {
 using namespace ptx;
 typedef __nv_bfloat16 bf16;
 
-constexpr int kTcThreads = 352;   // 11 warps
+constexpr int kTcThreads = 512;   // 16 warps
 constexpr int kTcDVT = 16;        // d_v columns per CTA
 constexpr int kGateBatch = 256;   // tokens per gate-warp batch
+
+#ifdef ESC_TC_TRACE   // bring-up only: per-chunk clock64() stamps of CTA (0,0), read back with esc_debug_trace_read
+__device__ long long g_tc_trace[16 * 64];
+#define TC_TRACE(ev, c) do { if (blockIdx.x == 0 && blockIdx.y == 0 && (c) < 64) g_tc_trace[(ev) * 64 + (c)] = clock64(); } while (0)
+#else
+#define TC_TRACE(ev, c) do { } while (0)
+#endif
 
 template <int DK, int C>
 struct TcCfg {
     static constexpr int NS = (C == 64) ? 3 : 2;          // input stages
     static constexpr int NB = (C == 64) ? 2 : 1;          // P / A / V~ buffers
+    static constexpr int NSB = (C == 64) ? 2 : 1;         // S operand buffers
+    static constexpr int SWA = (C == 64) ? 4 : 8;         // score-warp arrivals per chunk (one / both score groups)
     static constexpr int NH = DK / 64;                    // 64-column halves of a Q / K tile
     static constexpr int CPB = kGateBatch / C;            // chunks per gate batch
     static constexpr uint32_t half_bytes = C * 128;       // one [C x 64] bf16 half tile
@@ -56,10 +65,10 @@ struct TcCfg {
     static constexpr uint32_t stage_off = 0;
     static constexpr uint32_t a_off = stage_off + NS * stage_bytes;             // [NB][hi,lo]
     static constexpr uint32_t vt_off = a_off + NB * 2 * a_bytes;                // [NB][hi,lo]
-    static constexpr uint32_t s_off = vt_off + NB * 2 * vt_bytes;               // [hi,lo]
-    static constexpr uint32_t gate_off = s_off + 2 * s_bytes;                   // [2][b2[256], eb[256]] fp32
+    static constexpr uint32_t s_off = vt_off + NB * 2 * vt_bytes;               // [NSB][hi,lo]
+    static constexpr uint32_t gate_off = s_off + NSB * 2 * s_bytes;             // [2][b2[256], eb[256]] fp32
     static constexpr uint32_t bar_off = gate_off + 2 * 2 * kGateBatch * 4;
-    static constexpr uint32_t n_bars = 2 * NS + 4 * NB + 2 + 2 + 2 * 2 + 2 * 2 + 2 * 2;
+    static constexpr uint32_t n_bars = 2 * NS + 4 * NB + 2 * NSB + 2 * 2 + 2 * 2 + 2 * 2;
     static constexpr uint32_t total = bar_off + 64 * 8 + 16 + 1024;             // + alignment slack
     static constexpr uint32_t tmem_cols = 256;
     static constexpr uint32_t tm_p = 0;                    // [NB] x C columns
@@ -85,8 +94,8 @@ __device__ __forceinline__ constexpr TcBars tc_bars() {
     b.p_empty = i; i += L::NB;
     b.a_full = i; i += L::NB;
     b.a_empty = i; i += L::NB;
-    b.s_full = i; i += 1;
-    b.s_empty = i; i += 1;
+    b.s_full = i; i += L::NSB;
+    b.s_empty = i; i += L::NSB;
     b.o_full = i; i += 2;
     b.o_empty = i; i += 2;
     b.u_full = i; i += 2;
@@ -102,12 +111,9 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo_elem, float hi_elem) {   
 }
 // two-term split of a pair: returns packed hi terms, writes packed lo terms
 __device__ __forceinline__ uint32_t split2(float x0, float x1, uint32_t& lo) {
-    const bf16 h0 = __float2bfloat16_rn(x0), h1 = __float2bfloat16_rn(x1);
-    lo = pack_bf16(x0 - __bfloat162float(h0), x1 - __bfloat162float(h1));
-    __nv_bfloat162 p;
-    p.x = h0;
-    p.y = h1;
-    return *reinterpret_cast<uint32_t*>(&p);
+    const uint32_t hi = pack_bf16(x0, x1);   // one cvt.rn.bf16x2.f32
+    lo = pack_bf16(x0 - __uint_as_float(hi << 16), x1 - __uint_as_float(hi & 0xFFFF0000u));
+    return hi;
 }
 __device__ __forceinline__ float ex2(float x) {
     float y;
@@ -133,7 +139,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                    float* state_out, OutT* __restrict__ o, uint32_t H, uint32_t DV, uint64_t T, uint64_t t_stride) {
     using L = TcCfg<DK, C>;
     constexpr TcBars BI = tc_bars<DK, C>();
-    constexpr int NS = L::NS, NB = L::NB, CPB = L::CPB;
+    constexpr int NS = L::NS, NB = L::NB, NSB = L::NSB, SWA = L::SWA, CPB = L::CPB;
     constexpr uint32_t SBO_A = (C / 8) * 128, SBO_V = (C / 8) * 128, SBO_S = (DK / 8) * 128;
 
     extern __shared__ uint8_t smem_raw[];
@@ -150,16 +156,16 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
 
     // ---- one-time setup ----------------------------------------------------------------------------
     if (warp == 0 && lane == 0) {
-        for (int i = 0; i < NS; ++i) { mbar_init(&bars[BI.full + i], 1); mbar_init(&bars[BI.empty + i], 5); }
+        for (int i = 0; i < NS; ++i) { mbar_init(&bars[BI.full + i], 1); mbar_init(&bars[BI.empty + i], 1 + SWA); }
         for (int i = 0; i < NB; ++i) {
-            mbar_init(&bars[BI.p_full + i], 1); mbar_init(&bars[BI.p_empty + i], 4);
-            mbar_init(&bars[BI.a_full + i], 4); mbar_init(&bars[BI.a_empty + i], 1);
+            mbar_init(&bars[BI.p_full + i], 1); mbar_init(&bars[BI.p_empty + i], SWA);
+            mbar_init(&bars[BI.a_full + i], SWA); mbar_init(&bars[BI.a_empty + i], 1);
         }
-        mbar_init(&bars[BI.s_full], 4); mbar_init(&bars[BI.s_empty], 1);
+        for (int i = 0; i < NSB; ++i) { mbar_init(&bars[BI.s_full + i], 4); mbar_init(&bars[BI.s_empty + i], 1); }
         for (int i = 0; i < 2; ++i) {
             mbar_init(&bars[BI.o_full + i], 1); mbar_init(&bars[BI.o_empty + i], 4);
             mbar_init(&bars[BI.u_full + i], 1); mbar_init(&bars[BI.u_empty + i], 4);
-            mbar_init(&bars[BI.g_full + i], 1); mbar_init(&bars[BI.g_empty + i], 8);
+            mbar_init(&bars[BI.g_full + i], 1); mbar_init(&bars[BI.g_empty + i], 12);
         }
         fence_mbar_init();
         tma_prefetch_desc(&tq); tma_prefetch_desc(&tk); tma_prefetch_desc(&tv);
@@ -170,11 +176,11 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
         reinterpret_cast<uint4*>(sm + L::a_off)[i] = make_uint4(0, 0, 0, 0);
 
     // state warps own the carry: row `krow` of the [d_k x 16] slice per thread, fp32 registers
-    const bool st_warp = warp >= 7;
+    const bool st_warp = warp >= 12;
     const bool st_active = st_warp && (DK == 128 || lane < 16);
     const uint32_t krow = (DK == 128) ? 32 * q + lane : 16 * q + (lane & 15);
     float S[16];
-    auto write_s_operand = [&]() {   // S hi/lo as UMMA B operand, MN-major interleaved: (n,k) -> (n/8)*SBO + (k/8)*128 + (k%8)*16
+    auto write_s_operand = [&](uint32_t buf) {   // S hi/lo as UMMA B operand, MN-major interleaved: (n,k) -> (n/8)*SBO + (k/8)*128 + (k%8)*16
         if (st_active) {
 #pragma unroll
             for (int nb = 0; nb < 2; ++nb) {
@@ -184,8 +190,8 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 hi.z = split2(S[8 * nb + 4], S[8 * nb + 5], lo.z);
                 hi.w = split2(S[8 * nb + 6], S[8 * nb + 7], lo.w);
                 const uint32_t off = nb * SBO_S + (krow >> 3) * 128 + (krow & 7) * 16;
-                *reinterpret_cast<uint4*>(sm + L::s_off + off) = hi;
-                *reinterpret_cast<uint4*>(sm + L::s_off + L::s_bytes + off) = lo;
+                *reinterpret_cast<uint4*>(sm + L::s_off + buf * 2 * L::s_bytes + off) = hi;
+                *reinterpret_cast<uint4*>(sm + L::s_off + buf * 2 * L::s_bytes + L::s_bytes + off) = lo;
             }
         }
     };
@@ -200,7 +206,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 S[4 * j] = x.x; S[4 * j + 1] = x.y; S[4 * j + 2] = x.z; S[4 * j + 3] = x.w;
             }
         }
-        write_s_operand();
+        write_s_operand(0);
     }
     fence_proxy_async_smem();
     tc_fence_before_sync();
@@ -225,6 +231,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                     tma_load_4d(st + L::q_bytes + hh * L::half_bytes, &tk, full, hh * 64, (int)h, t0, (int)b);
                 }
                 tma_load_4d(st + 2 * L::q_bytes, &tv, full, (int)dv0, (int)h, t0, (int)b);
+                TC_TRACE(0, c);
             }
         }
     } else if (warp == 1) {
@@ -246,30 +253,15 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                                 smem_desc(ka + off, 16, 1024, kSwz128), idP, ks > 0);
                 }
                 mma_commit(&bars[BI.p_full + pb]);
+                TC_TRACE(1, c);
             };
-            auto issue_O1 = [&](uint32_t c) {
-                const uint32_t s = c % NS, ob = c & 1;
-                mbar_wait(&bars[BI.s_full], c & 1);
-                mbar_wait(&bars[BI.o_empty + ob], ((c >> 1) & 1) ^ 1);
-                tc_fence_after_sync();
-                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes;
-#pragma unroll
-                for (int term = 0; term < 2; ++term) {
-#pragma unroll
-                    for (int ks = 0; ks < DK / 16; ++ks) {
-                        const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
-                        mma_bf16_ss(tb + L::tm_o1 + ob * 16, smem_desc(qa + off, 16, 1024, kSwz128),
-                                    smem_desc(sm_a + L::s_off + term * L::s_bytes + 2 * ks * 128, 128, SBO_S, kSwzNone), idO,
-                                    (term | ks) > 0);
-                    }
-                }
-                mma_commit(&bars[BI.s_empty]);
-            };
-            auto issue_UO2 = [&](uint32_t c) {
+            auto issue_UO2 = [&](uint32_t c) {   // independent of the carried state: runs ahead of the chain
                 const uint32_t s = c % NS, pb = c % NB, ob = c & 1;
                 mbar_wait(&bars[BI.a_full + pb], (c / NB) & 1);
                 mbar_wait(&bars[BI.u_empty + ob], ((c >> 1) & 1) ^ 1);
+                mbar_wait(&bars[BI.o_empty + ob], ((c >> 1) & 1) ^ 1);
                 tc_fence_after_sync();
+                TC_TRACE(2, c);
                 const uint32_t ka = sm_a + L::stage_off + s * L::stage_bytes + L::q_bytes, va = ka + L::q_bytes;
                 const uint32_t vt = sm_a + L::vt_off + pb * 2 * L::vt_bytes, aa = sm_a + L::a_off + pb * 2 * L::a_bytes;
 #pragma unroll
@@ -287,15 +279,33 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                         mma_bf16_ss(tb + L::tm_o2 + ob * 16, smem_desc(aa + term * L::a_bytes + 2 * ks * 128, 128, SBO_A, kSwzNone),
                                     smem_desc(va + 2 * ks * 256, 512, 256, kSwz32), idO, (term | ks) > 0);
                 }
-                mma_commit(&bars[BI.o_full + ob]);
                 mma_commit(&bars[BI.a_empty + pb]);
-                mma_commit(&bars[BI.empty + s]);
+            };
+            auto issue_O1 = [&](uint32_t c) {    // the only MMA that reads the carried state (version c of the S operand)
+                const uint32_t s = c % NS, ob = c & 1, sb = c % NSB;
+                mbar_wait(&bars[BI.s_full + sb], (c / NSB) & 1);
+                tc_fence_after_sync();
+                TC_TRACE(3, c);
+                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes;
+                const uint32_t sa = sm_a + L::s_off + sb * 2 * L::s_bytes;
+#pragma unroll
+                for (int term = 0; term < 2; ++term) {
+#pragma unroll
+                    for (int ks = 0; ks < DK / 16; ++ks) {
+                        const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
+                        mma_bf16_ss(tb + L::tm_o1 + ob * 16, smem_desc(qa + off, 16, 1024, kSwz128),
+                                    smem_desc(sa + term * L::s_bytes + 2 * ks * 128, 128, SBO_S, kSwzNone), idO, (term | ks) > 0);
+                    }
+                }
+                mma_commit(&bars[BI.s_empty + sb]);
+                mma_commit(&bars[BI.o_full + ob]);   // O1(c) and O2(c) (issued earlier) are both complete
+                mma_commit(&bars[BI.empty + s]);     // last reader of stage s
             };
             if (n_chunks) issue_P(0);
             for (uint32_t c = 0; c < n_chunks; ++c) {
                 if (c + 1 < n_chunks) issue_P(c + 1);   // keeps the tensor pipe busy while the score warps build A(c)
-                issue_O1(c);
                 issue_UO2(c);
+                issue_O1(c);
             }
         }
     } else if (warp == 2) {
@@ -341,21 +351,26 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             if (lane == 0) mbar_arrive(&bars[BI.g_full + slot]);
         }
     }
-    else if (warp < 7) {
+    else if (warp >= 4 && warp < 12) {
         // ================= score warps: A = P ⊙ 2^(b_i - b_j) (causal), V~ = V ⊙ 2^(b_C - b_j) =================
-        const int tid_wg = (warp - 3) * 32 + lane;
-        constexpr int NG = C / 64;                 // 16-row groups per warp (row r of an M=64 tile sits in lane 32(r/16)+r%16)
-        for (uint32_t c = 0; c < n_chunks; ++c) {
+        // two groups of 4 warps (one warp per TMEM lane quadrant).  C = 64: the groups alternate chunks (and own the
+        // P / A / V~ buffer of their parity).  C = 128: both groups work on every chunk, one 16-row group per quadrant each.
+        const uint32_t wg = (uint32_t)(warp - 4) >> 2;
+        constexpr bool kAlt = (C == 64);
+        const int tid_s = kAlt ? ((warp - 4) & 3) * 32 + lane : (warp - 4) * 32 + lane;   // index among the threads sharing a chunk
+        constexpr int kSThreads = kAlt ? 128 : 256;
+        for (uint32_t c = kAlt ? wg : 0; c < n_chunks; c += kAlt ? 2 : 1) {
             const uint32_t s = c % NS, pb = c % NB, bt = c / CPB, gslot = bt & 1;
             mbar_wait(&bars[BI.g_full + gslot], (bt >> 1) & 1);
             const float* b2 = gate + gslot * 2 * kGateBatch + (c % CPB) * C;
             mbar_wait(&bars[BI.full + s], (c / NS) & 1);
             mbar_wait(&bars[BI.a_empty + pb], ((c / NB) & 1) ^ 1);
+            if (q == 3 && lane == 0) TC_TRACE(10, c);
             {   // V~ hi/lo, UMMA B operand MN-major interleaved: (n,k=token) -> (n/8)*SBO_V + (k/8)*128 + (k%8)*16 + (n%8)*2
                 const uint8_t* vs = sm + L::stage_off + s * L::stage_bytes + 2 * L::q_bytes;
                 uint8_t* vt = sm + L::vt_off + pb * 2 * L::vt_bytes;
                 const float b_last = b2[C - 1];
-                for (int idx = tid_wg; idx < C * 2; idx += 128) {
+                for (int idx = tid_s; idx < C * 2; idx += kSThreads) {
                     const int j = idx >> 1, half = idx & 1;
                     const uint4 raw = *reinterpret_cast<const uint4*>(vs + j * 32 + ((half ^ ((j >> 2) & 1)) * 16));   // undo 32B swizzle
                     const float sc = ex2(b_last - b2[j]);
@@ -373,23 +388,25 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             }
             mbar_wait(&bars[BI.p_full + pb], (c / NB) & 1);
             tc_fence_after_sync();
+            if (q == 3 && lane == 0) TC_TRACE(4, c);
             uint8_t* ah = sm + L::a_off + pb * 2 * L::a_bytes;
-#pragma unroll
-            for (int gi = 0; gi < NG; ++gi) {
-                const int rg = (C == 64) ? q : 2 * q + gi;             // 16-row group index
-                const uint32_t lane_base = (C == 64) ? 32 * q : 32 * q + 16 * gi;
+            {
+                // 16-row group of this warp: row r of an M=64 tile sits in TMEM lane 32(r/16) + r%16, of an M=128 tile in lane r
+                const int rg = kAlt ? q : 2 * q + (int)wg;
+                const uint32_t lane_base = kAlt ? 32 * q : 32 * q + 16 * wg;
                 uint32_t r[C / 16][8];
 #pragma unroll
                 for (int cb = 0; cb < C / 16; ++cb)
                     if (cb <= rg) tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_p + pb * C + cb * 16), r[cb]);
                 tmem_ld_wait();
-                if (gi == NG - 1) {   // P(c) is in registers: the MMA thread may overwrite this TMEM buffer
-                    tc_fence_before_sync();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(&bars[BI.p_empty + pb]);
-                }
+                tc_fence_before_sync();   // P(c) is in registers: the MMA thread may overwrite this TMEM buffer
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bars[BI.p_empty + pb]);
+                if (q == 3 && lane == 0) TC_TRACE(11, c);
                 const int ra = 16 * rg + (lane >> 2), rb = ra + 8;
                 const float ba = b2[ra], bb = b2[rb];
+                // UMMA A operand, K-major interleaved: (i,j) -> (i/8)*SBO_A + (j/8)*128 + (i%8)*16 + (j%8)*2
+                uint8_t* arow = ah + (ra >> 3) * SBO_A + (ra & 7) * 16 + (lane & 3) * 4;
 #pragma unroll
                 for (int cb = 0; cb < C / 16; ++cb) {
                     if (cb <= rg) {
@@ -409,26 +426,27 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                             }
                             uint32_t lo_a, lo_c;
                             const uint32_t hi_a = split2(a0, a1, lo_a), hi_c = split2(c0, c1, lo_c);
-                            // UMMA A operand, K-major interleaved: (i,j) -> (i/8)*SBO_A + (j/8)*128 + (i%8)*16 + (j%8)*2
-                            const uint32_t oa = (ra >> 3) * SBO_A + (j0 >> 3) * 128 + (ra & 7) * 16 + (j0 & 7) * 2;
-                            const uint32_t oc = (rb >> 3) * SBO_A + (j0 >> 3) * 128 + (rb & 7) * 16 + (j0 & 7) * 2;
-                            *reinterpret_cast<uint32_t*>(ah + oa) = hi_a;
-                            *reinterpret_cast<uint32_t*>(ah + L::a_bytes + oa) = lo_a;
-                            *reinterpret_cast<uint32_t*>(ah + oc) = hi_c;
-                            *reinterpret_cast<uint32_t*>(ah + L::a_bytes + oc) = lo_c;
+                            uint8_t* pa = arow + (cb * 2 + jb) * 128;
+                            *reinterpret_cast<uint32_t*>(pa) = hi_a;
+                            *reinterpret_cast<uint32_t*>(pa + L::a_bytes) = lo_a;
+                            *reinterpret_cast<uint32_t*>(pa + SBO_A) = hi_c;              // row + 8
+                            *reinterpret_cast<uint32_t*>(pa + SBO_A + L::a_bytes) = lo_c;
                         }
                     }
                 }
             }
             fence_proxy_async_smem();   // generic-proxy writes of A, V~ -> visible to tcgen05.mma's operand reads
             __syncwarp();
+            if (q == 3 && lane == 0) TC_TRACE(5, c);
             if (lane == 0) {
                 mbar_arrive(&bars[BI.a_full + pb]);
                 mbar_arrive(&bars[BI.empty + s]);
-                if ((c % CPB) == CPB - 1 || c + 1 == n_chunks) mbar_arrive(&bars[BI.g_empty + gslot]);
+                const bool last_in_batch = kAlt ? ((c % CPB) + 2 >= (uint32_t)CPB || c + 2 >= n_chunks)
+                                                : ((c % CPB) == (uint32_t)CPB - 1 || c + 1 == n_chunks);
+                if (last_in_batch) mbar_arrive(&bars[BI.g_empty + gslot]);
             }
         }
-    } else {
+    } else if (warp >= 12) {
         // ================= state warps: carry S, emit o =================
         constexpr int NG = C / 64;
         for (uint32_t c = 0; c < n_chunks; ++c) {
@@ -438,6 +456,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             // ---- the carry: S <- 2^(b_C) S + U, fp32 FMA in registers ----
             mbar_wait(&bars[BI.u_full + ob], (c >> 1) & 1);
             tc_fence_after_sync();
+            if (q == 3 && lane == 0) TC_TRACE(6, c);
             uint32_t ur[16];
             tmem_ld_32x32b_x16(tmem_addr(tb, 32 * q, L::tm_u + ob * 16), ur);
             tmem_ld_wait();
@@ -447,16 +466,19 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             const float gam = eb[C - 1];
 #pragma unroll
             for (int j = 0; j < 16; ++j) S[j] = fmaf(gam, S[j], __uint_as_float(ur[j]));
-            if (c + 1 < n_chunks) {
-                mbar_wait(&bars[BI.s_empty], c & 1);   // O1(c) has finished reading the previous operand
-                write_s_operand();
+            if (c + 1 < n_chunks) {   // version c+1 of the S operand (read by O1(c+1))
+                const uint32_t sb = (c + 1) % NSB;
+                mbar_wait(&bars[BI.s_empty + sb], ((((c + 1) / NSB) & 1) ^ 1));
+                write_s_operand(sb);
                 fence_proxy_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&bars[BI.s_full]);
+                if (lane == 0) mbar_arrive(&bars[BI.s_full + sb]);
             }
+            if (q == 3 && lane == 0) TC_TRACE(7, c);
             // ---- epilogue: o_i = 2^(b_i) O1_i + O2_i ----
             mbar_wait(&bars[BI.o_full + ob], (c >> 1) & 1);
             tc_fence_after_sync();
+            if (q == 3 && lane == 0) TC_TRACE(8, c);
             const uint64_t t0 = (uint64_t)c * C;
             const int n = (int)((T - t0) < (uint64_t)C ? (T - t0) : (uint64_t)C);
 #pragma unroll
@@ -487,6 +509,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 }
             }
             __syncwarp();
+            if (q == 3 && lane == 0) TC_TRACE(9, c);
             if (lane == 0 && ((c % CPB) == CPB - 1 || c + 1 == n_chunks)) mbar_arrive(&bars[BI.g_empty + gslot]);
         }
         if (st_active) {
@@ -575,5 +598,11 @@ int launch_scan_tc(const ScanShape& s, const void* q, const void* k, const void*
     if (s.dk == 64 && s.chunk == 128) return launch_tc_o<64, 128>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
     return ESC_ERR_UNSUPPORTED;
 }
+
+#ifdef ESC_TC_TRACE
+extern "C" int esc_debug_trace_read(long long* host) {
+    return (int)cudaMemcpyFromSymbol(host, g_tc_trace, sizeof(g_tc_trace));
+}
+#endif
 
 }  // namespace esc
