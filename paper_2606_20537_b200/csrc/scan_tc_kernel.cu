@@ -3,27 +3,31 @@
 // Definition (BASELINE.json north_star; "a fold over the entire prefix", folded "per
 // chunk" PAPER.md:169):   S_t = g_t S_{t-1} + k_t^T v_t ,  o_t = q_t S_t.
 // Chunk algebra (exact-arithmetic equivalent; every exponent <= 0), with b_i = sum_{r<=i} log2 g_r:
-//     P      = Q K^T                                  (C x C)        tcgen05.mma  M=C  N=C  K=d_k
+//     P      = Q K^T                                  (C x C)     tcgen05.mma  M=C   N=C   K=d_k
 //     A_ij   = P_ij 2^(b_i - b_j) [j <= i]            fp32 ALU + MUFU, split into bf16 hi + lo
-//     O1     = Q S_prev                               (C x 16)       tcgen05.mma  (S_prev hi + lo)
-//     O2     = A V                                    (C x 16)       tcgen05.mma  (A hi + lo)
-//     o_i    = 2^(b_i) O1_i + O2_i                    fp32 epilogue
-//     U      = K^T V~ ,  V~_j = 2^(b_C - b_j) v_j     (d_k x 16)     tcgen05.mma  (V~ hi + lo)
-//     S_next = 2^(b_C) S_prev + U                     fp32 FMA in registers (the carry chain)
+//     O1     = Q [S_hi | S_lo]                        (C x 32)    tcgen05.mma  M=C   N=32  K=d_k
+//     O2     = A_hi V + A_lo V                        (C x 16)    tcgen05.mma  M=C   N=16  K=C  (x2)
+//     o_i    = 2^(b_i) (O1h_i + O1l_i) + O2_i         fp32 epilogue
+//     U      = K^T [V~_hi | V~_lo] , V~_j = 2^(b_C - b_j) v_j   (d_k x 32)  tcgen05.mma  M=d_k N=32 K=C
+//     S_next = 2^(b_C) S_prev + (Uh + Ul)             fp32 FMA in registers (the carry chain)
 //
 // One CTA owns (b, h, 16 columns of d_v) — the columns of S are independent — and walks the chunks
-// in order.  Only the last line is a true dependency between chunks: P, A, O2, U of later chunks do
-// not depend on S, so the kernel is a software pipeline of specialised warps
-//   warp 0      TMA producer: Q / K / V chunk tiles -> 128B/32B-swizzled shared memory, NS-stage ring
-//   warp 1      MMA issuer: one thread issues every tcgen05.mma; accumulators live in TMEM
-//   warp 2      gate warp: log2 g, segmented warp-shuffle prefix sums for 256 tokens at a time
-//   warps 4-11  score warps (2 groups): P (TMEM) -> A hi/lo (smem, UMMA K-major interleaved), V -> V~ hi/lo
-//   warps 12-15 state warps: U (TMEM) -> carry S in registers -> S hi/lo operand; O1,O2 -> o (global)
-// synchronised only by mbarriers (TMA complete_tx, tcgen05.commit, warp arrivals).
+// in order.  Only the last line is a true dependency between chunks, and only O1 reads the carried
+// state, so the kernel is a software pipeline of specialised warps synchronised by mbarriers only:
+//   warp 0       TMA producer: Q / K / V chunk tiles -> 128B/32B-swizzled smem ring (+ L2 prefetch ahead)
+//   warp 1       gate warp: log2 g, segmented warp-shuffle prefix sums, 256 tokens per batch
+//   warps 2,3,20,21  MMA issuers, one thread each: P | O1 | U | O2.  A tcgen05.mma costs its issuing
+//                thread ~55 cycles whatever its shape (measured), the tensor pipe only max(23, M'N/256):
+//                four issuers keep the pipe, not the issue slot, the limit, and give every product its
+//                own dependency chain (no head-of-line blocking behind the state-dependent O1)
+//   warps 4-11   score warps (2 groups): P (TMEM) -> A hi/lo (smem, UMMA K-major interleaved), V -> V~
+//   warps 12-15  state warps: U (TMEM) -> carry S in fp32 registers -> [S_hi | S_lo] operand
+//   warps 16-19  epilogue warps: O1, O2 (TMEM) -> o (global)
 //
 // Bit-identity: the carry is a pure function of (S_prev bits, chunk inputs); there
-// is no T-dependent tiling, no atomics, no split-K; the MMA issue order inside a chunk is fixed.
-// Precision: raw Q, K, V are bf16 inputs; A, V~, S_prev are two-term bf16 splits.
+// is no T-dependent tiling, no atomics, no split-K; every accumulator is produced by ONE issuer thread
+// in a fixed order.  Precision: raw Q, K, V are the bf16 inputs; A, V~, S_prev are
+// two-term bf16 splits (hi + lo), the hi|lo halves of V~ and S ride in one MMA as 32 columns.
 #include <cuda.h>
 #include <cuda_bf16.h>
 
@@ -35,9 +39,12 @@ namespace esc {
 using namespace ptx;
 typedef __nv_bfloat16 bf16;
 
-constexpr int kTcThreads = 512;   // 16 warps
+constexpr int kTcWarps = 22;
+constexpr int kTcThreads = kTcWarps * 32;
 constexpr int kTcDVT = 16;        // d_v columns per CTA
+constexpr int kTcNM = 2 * kTcDVT; // columns of a merged hi|lo operand
 constexpr int kGateBatch = 256;   // tokens per gate-warp batch
+constexpr int kPrefetchAhead = 6; // chunks the producer prefetches into L2 ahead of its smem ring
 
 #ifdef ESC_TC_TRACE   // bring-up only: per-chunk clock64() stamps of CTA (0,0), read back with esc_debug_trace_read
 __device__ long long g_tc_trace[16 * 64];
@@ -48,7 +55,7 @@ __device__ long long g_tc_trace[16 * 64];
 
 template <int DK, int C>
 struct TcCfg {
-    static constexpr int NS = (C == 64) ? 3 : 2;          // input stages
+    static constexpr int NS = (C == 64) ? 4 : 2;          // input stages
     static constexpr int NB = (C == 64) ? 2 : 1;          // P / A / V~ buffers
     static constexpr int NSB = (C == 64) ? 2 : 1;         // S operand buffers
     static constexpr int SWA = (C == 64) ? 4 : 8;         // score-warp arrivals per chunk (one / both score groups)
@@ -59,29 +66,31 @@ struct TcCfg {
     static constexpr uint32_t v_bytes = C * 32;           // [C x 16] bf16
     static constexpr uint32_t stage_bytes = 2 * q_bytes + v_bytes;   // multiple of 1024
     static constexpr uint32_t a_bytes = C * C * 2;        // one A term
-    static constexpr uint32_t vt_bytes = C * kTcDVT * 2;  // one V~ term
-    static constexpr uint32_t s_bytes = DK * kTcDVT * 2;  // one S term
+    static constexpr uint32_t vt_bytes = C * kTcNM * 2;   // merged V~ operand [32 x C]
+    static constexpr uint32_t s_bytes = DK * kTcNM * 2;   // merged S operand [32 x DK]
     // offsets from the 1024-aligned base
     static constexpr uint32_t stage_off = 0;
     static constexpr uint32_t a_off = stage_off + NS * stage_bytes;             // [NB][hi,lo]
-    static constexpr uint32_t vt_off = a_off + NB * 2 * a_bytes;                // [NB][hi,lo]
-    static constexpr uint32_t s_off = vt_off + NB * 2 * vt_bytes;               // [NSB][hi,lo]
-    static constexpr uint32_t gate_off = s_off + NSB * 2 * s_bytes;             // [2][b2[256], eb[256]] fp32
+    static constexpr uint32_t vt_off = a_off + NB * 2 * a_bytes;                // [NB]
+    static constexpr uint32_t s_off = vt_off + NB * vt_bytes;                   // [NSB]
+    static constexpr uint32_t gate_off = s_off + NSB * s_bytes;                 // [2][b2[256], eb[256]] fp32
     static constexpr uint32_t bar_off = gate_off + 2 * 2 * kGateBatch * 4;
-    static constexpr uint32_t n_bars = 2 * NS + 4 * NB + 2 * NSB + 2 * 2 + 2 * 2 + 2 * 2;
+    static constexpr uint32_t n_bars = 2 * NS + 4 * NB + 2 * NSB + 14;
     static constexpr uint32_t total = bar_off + 64 * 8 + 16 + 1024;             // + alignment slack
-    static constexpr uint32_t tmem_cols = 256;
+    static constexpr uint32_t tmem_cols = 512;
     static constexpr uint32_t tm_p = 0;                    // [NB] x C columns
-    static constexpr uint32_t tm_u = NB * C;               // [2] x 16
-    static constexpr uint32_t tm_o1 = tm_u + 32;           // [2] x 16
-    static constexpr uint32_t tm_o2 = tm_o1 + 32;          // [2] x 16
+    static constexpr uint32_t tm_u = NB * C;               // [2] x 32
+    static constexpr uint32_t tm_o1 = tm_u + 64;           // [2] x 32
+    static constexpr uint32_t tm_o2 = tm_o1 + 64;          // [2] x 16
     static_assert(tm_o2 + 32 <= tmem_cols, "TMEM budget");
     static_assert(stage_bytes % 1024 == 0, "stages must keep 1024-byte alignment (128B swizzle)");
     static_assert(n_bars <= 64, "barrier area");
+    static_assert(total <= 232448, "shared memory budget");
 };
 
 struct TcBars {   // indices into the mbarrier array
-    int full, empty, p_full, p_empty, a_full, a_empty, s_full, s_empty, o_full, o_empty, u_full, u_empty, g_full, g_empty;
+    int full, empty, p_full, p_empty, a_full, a_empty, s_full, s_empty, o1_full, o2_full, o_empty, u_full, u_empty, g_full,
+        g_empty;
 };
 template <int DK, int C>
 __device__ __forceinline__ constexpr TcBars tc_bars() {
@@ -96,7 +105,8 @@ __device__ __forceinline__ constexpr TcBars tc_bars() {
     b.a_empty = i; i += L::NB;
     b.s_full = i; i += L::NSB;
     b.s_empty = i; i += L::NSB;
-    b.o_full = i; i += 2;
+    b.o1_full = i; i += 2;
+    b.o2_full = i; i += 2;
     b.o_empty = i; i += 2;
     b.u_full = i; i += 2;
     b.u_empty = i; i += 2;
@@ -156,32 +166,35 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
 
     // ---- one-time setup ----------------------------------------------------------------------------
     if (warp == 0 && lane == 0) {
-        for (int i = 0; i < NS; ++i) { mbar_init(&bars[BI.full + i], 1); mbar_init(&bars[BI.empty + i], 1 + SWA); }
+        for (int i = 0; i < NS; ++i) { mbar_init(&bars[BI.full + i], 1); mbar_init(&bars[BI.empty + i], 4 + SWA); }
         for (int i = 0; i < NB; ++i) {
             mbar_init(&bars[BI.p_full + i], 1); mbar_init(&bars[BI.p_empty + i], SWA);
-            mbar_init(&bars[BI.a_full + i], SWA); mbar_init(&bars[BI.a_empty + i], 1);
+            mbar_init(&bars[BI.a_full + i], SWA); mbar_init(&bars[BI.a_empty + i], 2);
         }
         for (int i = 0; i < NSB; ++i) { mbar_init(&bars[BI.s_full + i], 4); mbar_init(&bars[BI.s_empty + i], 1); }
         for (int i = 0; i < 2; ++i) {
-            mbar_init(&bars[BI.o_full + i], 1); mbar_init(&bars[BI.o_empty + i], 4);
+            mbar_init(&bars[BI.o1_full + i], 1); mbar_init(&bars[BI.o2_full + i], 1); mbar_init(&bars[BI.o_empty + i], 4);
             mbar_init(&bars[BI.u_full + i], 1); mbar_init(&bars[BI.u_empty + i], 4);
-            mbar_init(&bars[BI.g_full + i], 1); mbar_init(&bars[BI.g_empty + i], 12);
+            mbar_init(&bars[BI.g_full + i], 1); mbar_init(&bars[BI.g_empty + i], 16);
         }
         fence_mbar_init();
         tma_prefetch_desc(&tq); tma_prefetch_desc(&tk); tma_prefetch_desc(&tv);
     }
-    if (warp == 1) tmem_alloc(tmem_slot, L::tmem_cols);
+    if (warp == 2) tmem_alloc(tmem_slot, L::tmem_cols);
     // A buffers: the strictly-upper 16x16 blocks are never written again and must read as zero
     for (uint32_t i = threadIdx.x; i < NB * 2 * L::a_bytes / 16; i += kTcThreads)
         reinterpret_cast<uint4*>(sm + L::a_off)[i] = make_uint4(0, 0, 0, 0);
 
     // state warps own the carry: row `krow` of the [d_k x 16] slice per thread, fp32 registers
-    const bool st_warp = warp >= 12;
+    const bool st_warp = warp >= 12 && warp < 16;
     const bool st_active = st_warp && (DK == 128 || lane < 16);
     const uint32_t krow = (DK == 128) ? 32 * q + lane : 16 * q + (lane & 15);
     float S[16];
-    auto write_s_operand = [&](uint32_t buf) {   // S hi/lo as UMMA B operand, MN-major interleaved: (n,k) -> (n/8)*SBO + (k/8)*128 + (k%8)*16
+    // [S_hi | S_lo] as UMMA B operand, MN-major interleaved: (n,k) -> (n/8)*SBO_S + (k/8)*128 + (k%8)*16 + (n%8)*2,
+    // columns n = 0..15 hold the hi terms, 16..31 the lo terms
+    auto write_s_operand = [&](uint32_t buf) {
         if (st_active) {
+            uint8_t* base = sm + L::s_off + buf * L::s_bytes + (krow >> 3) * 128 + (krow & 7) * 16;
 #pragma unroll
             for (int nb = 0; nb < 2; ++nb) {
                 uint4 hi, lo;
@@ -189,9 +202,8 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 hi.y = split2(S[8 * nb + 2], S[8 * nb + 3], lo.y);
                 hi.z = split2(S[8 * nb + 4], S[8 * nb + 5], lo.z);
                 hi.w = split2(S[8 * nb + 6], S[8 * nb + 7], lo.w);
-                const uint32_t off = nb * SBO_S + (krow >> 3) * 128 + (krow & 7) * 16;
-                *reinterpret_cast<uint4*>(sm + L::s_off + buf * 2 * L::s_bytes + off) = hi;
-                *reinterpret_cast<uint4*>(sm + L::s_off + buf * 2 * L::s_bytes + L::s_bytes + off) = lo;
+                *reinterpret_cast<uint4*>(base + nb * SBO_S) = hi;
+                *reinterpret_cast<uint4*>(base + (2 + nb) * SBO_S) = lo;
             }
         }
     };
@@ -218,8 +230,21 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     if (warp == 0) {
         // ================= TMA producer =================
         if (lane == 0) {
+            auto prefetch = [&](uint32_t c) {   // pull chunk c's tiles into L2 (Q, K once per head: by the dv-slice-0 CTA)
+                const int t0 = (int)(c * C);
+                if (blockIdx.x == 0) {
+#pragma unroll
+                    for (int hh = 0; hh < L::NH; ++hh) {
+                        tma_prefetch_4d(&tq, hh * 64, (int)h, t0, (int)b);
+                        tma_prefetch_4d(&tk, hh * 64, (int)h, t0, (int)b);
+                    }
+                }
+                tma_prefetch_4d(&tv, (int)dv0, (int)h, t0, (int)b);
+            };
+            for (uint32_t c = NS; c < n_chunks && c < NS + kPrefetchAhead; ++c) prefetch(c);
             for (uint32_t c = 0; c < n_chunks; ++c) {
                 const uint32_t s = c % NS;
+                if (c + NS + kPrefetchAhead < n_chunks) prefetch(c + NS + kPrefetchAhead);
                 mbar_wait(&bars[BI.empty + s], ((c / NS) & 1) ^ 1);
                 uint8_t* st = sm + L::stage_off + s * L::stage_bytes;
                 uint64_t* full = &bars[BI.full + s];
@@ -235,80 +260,6 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             }
         }
     } else if (warp == 1) {
-        // ================= MMA issuer (one thread) =================
-        if (lane == 0) {
-            constexpr uint32_t idP = idesc_bf16(C, C, 0, 0);
-            constexpr uint32_t idO = idesc_bf16(C, kTcDVT, 0, 1);
-            constexpr uint32_t idU = idesc_bf16(DK, kTcDVT, 1, 1);
-            auto issue_P = [&](uint32_t c) {
-                const uint32_t s = c % NS, pb = c % NB;
-                mbar_wait(&bars[BI.full + s], (c / NS) & 1);
-                mbar_wait(&bars[BI.p_empty + pb], ((c / NB) & 1) ^ 1);
-                tc_fence_after_sync();
-                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes, ka = qa + L::q_bytes;
-#pragma unroll
-                for (int ks = 0; ks < DK / 16; ++ks) {
-                    const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
-                    mma_bf16_ss(tb + L::tm_p + pb * C, smem_desc(qa + off, 16, 1024, kSwz128),
-                                smem_desc(ka + off, 16, 1024, kSwz128), idP, ks > 0);
-                }
-                mma_commit(&bars[BI.p_full + pb]);
-                TC_TRACE(1, c);
-            };
-            auto issue_UO2 = [&](uint32_t c) {   // independent of the carried state: runs ahead of the chain
-                const uint32_t s = c % NS, pb = c % NB, ob = c & 1;
-                mbar_wait(&bars[BI.a_full + pb], (c / NB) & 1);
-                mbar_wait(&bars[BI.u_empty + ob], ((c >> 1) & 1) ^ 1);
-                mbar_wait(&bars[BI.o_empty + ob], ((c >> 1) & 1) ^ 1);
-                tc_fence_after_sync();
-                TC_TRACE(2, c);
-                const uint32_t ka = sm_a + L::stage_off + s * L::stage_bytes + L::q_bytes, va = ka + L::q_bytes;
-                const uint32_t vt = sm_a + L::vt_off + pb * 2 * L::vt_bytes, aa = sm_a + L::a_off + pb * 2 * L::a_bytes;
-#pragma unroll
-                for (int term = 0; term < 2; ++term) {   // U = K^T V~ : A operand = the K tile read MN-major
-#pragma unroll
-                    for (int ks = 0; ks < C / 16; ++ks)
-                        mma_bf16_ss(tb + L::tm_u + ob * 16, smem_desc(ka + 2 * ks * 1024, L::half_bytes, 1024, kSwz128),
-                                    smem_desc(vt + term * L::vt_bytes + 2 * ks * 128, 128, SBO_V, kSwzNone), idU, (term | ks) > 0);
-                }
-                mma_commit(&bars[BI.u_full + ob]);
-#pragma unroll
-                for (int term = 0; term < 2; ++term) {   // O2 = A V : B operand = the V tile read MN-major (32B swizzle)
-#pragma unroll
-                    for (int ks = 0; ks < C / 16; ++ks)
-                        mma_bf16_ss(tb + L::tm_o2 + ob * 16, smem_desc(aa + term * L::a_bytes + 2 * ks * 128, 128, SBO_A, kSwzNone),
-                                    smem_desc(va + 2 * ks * 256, 512, 256, kSwz32), idO, (term | ks) > 0);
-                }
-                mma_commit(&bars[BI.a_empty + pb]);
-            };
-            auto issue_O1 = [&](uint32_t c) {    // the only MMA that reads the carried state (version c of the S operand)
-                const uint32_t s = c % NS, ob = c & 1, sb = c % NSB;
-                mbar_wait(&bars[BI.s_full + sb], (c / NSB) & 1);
-                tc_fence_after_sync();
-                TC_TRACE(3, c);
-                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes;
-                const uint32_t sa = sm_a + L::s_off + sb * 2 * L::s_bytes;
-#pragma unroll
-                for (int term = 0; term < 2; ++term) {
-#pragma unroll
-                    for (int ks = 0; ks < DK / 16; ++ks) {
-                        const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
-                        mma_bf16_ss(tb + L::tm_o1 + ob * 16, smem_desc(qa + off, 16, 1024, kSwz128),
-                                    smem_desc(sa + term * L::s_bytes + 2 * ks * 128, 128, SBO_S, kSwzNone), idO, (term | ks) > 0);
-                    }
-                }
-                mma_commit(&bars[BI.s_empty + sb]);
-                mma_commit(&bars[BI.o_full + ob]);   // O1(c) and O2(c) (issued earlier) are both complete
-                mma_commit(&bars[BI.empty + s]);     // last reader of stage s
-            };
-            if (n_chunks) issue_P(0);
-            for (uint32_t c = 0; c < n_chunks; ++c) {
-                if (c + 1 < n_chunks) issue_P(c + 1);   // keeps the tensor pipe busy while the score warps build A(c)
-                issue_UO2(c);
-                issue_O1(c);
-            }
-        }
-    } else if (warp == 2) {
         // ================= gate warp: b2_i = sum_{r<=i in chunk} log2 g_r, 256 tokens per batch =================
         const uint32_t n_batches = (uint32_t)((T + kGateBatch - 1) / kGateBatch);
         constexpr int GL = C / 8;   // lanes per chunk
@@ -350,6 +301,95 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars[BI.g_full + slot]);
         }
+    } else if (warp == 2) {
+        // ================= issuer: P = Q K^T =================
+        if (lane == 0) {
+            constexpr uint32_t idP = idesc_bf16(C, C, 0, 0);
+            for (uint32_t c = 0; c < n_chunks; ++c) {
+                const uint32_t s = c % NS, pb = c % NB;
+                mbar_wait(&bars[BI.full + s], (c / NS) & 1);
+                mbar_wait(&bars[BI.p_empty + pb], ((c / NB) & 1) ^ 1);
+                tc_fence_after_sync();
+                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes, ka = qa + L::q_bytes;
+#pragma unroll
+                for (int ks = 0; ks < DK / 16; ++ks) {
+                    const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
+                    mma_bf16_ss(tb + L::tm_p + pb * C, smem_desc(qa + off, 16, 1024, kSwz128),
+                                smem_desc(ka + off, 16, 1024, kSwz128), idP, ks > 0);
+                }
+                mma_commit(&bars[BI.p_full + pb]);
+                mma_commit(&bars[BI.empty + s]);
+                TC_TRACE(1, c);
+            }
+        }
+    } else if (warp == 3) {
+        // ================= issuer: O1 = Q [S_hi | S_lo] — the only MMA that reads the carried state =================
+        if (lane == 0) {
+            constexpr uint32_t idO1 = idesc_bf16(C, kTcNM, 0, 1);
+            for (uint32_t c = 0; c < n_chunks; ++c) {
+                const uint32_t s = c % NS, ob = c & 1, sb = c % NSB;
+                mbar_wait(&bars[BI.full + s], (c / NS) & 1);
+                mbar_wait(&bars[BI.o_empty + ob], ((c >> 1) & 1) ^ 1);
+                mbar_wait(&bars[BI.s_full + sb], (c / NSB) & 1);
+                tc_fence_after_sync();
+                TC_TRACE(2, c);
+                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes, sa = sm_a + L::s_off + sb * L::s_bytes;
+#pragma unroll
+                for (int ks = 0; ks < DK / 16; ++ks) {
+                    const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
+                    mma_bf16_ss(tb + L::tm_o1 + ob * 32, smem_desc(qa + off, 16, 1024, kSwz128),
+                                smem_desc(sa + 2 * ks * 128, 128, SBO_S, kSwzNone), idO1, ks > 0);
+                }
+                mma_commit(&bars[BI.s_empty + sb]);
+                mma_commit(&bars[BI.o1_full + ob]);
+                mma_commit(&bars[BI.empty + s]);
+            }
+        }
+    } else if (warp == 20) {
+        // ================= issuer: U = K^T [V~_hi | V~_lo] (A operand = the K tile read MN-major) =================
+        if (lane == 0) {
+            constexpr uint32_t idU = idesc_bf16(DK, kTcNM, 1, 1);
+            for (uint32_t c = 0; c < n_chunks; ++c) {
+                const uint32_t s = c % NS, pb = c % NB, ob = c & 1;
+                mbar_wait(&bars[BI.full + s], (c / NS) & 1);
+                mbar_wait(&bars[BI.u_empty + ob], ((c >> 1) & 1) ^ 1);
+                mbar_wait(&bars[BI.a_full + pb], (c / NB) & 1);
+                tc_fence_after_sync();
+                TC_TRACE(3, c);
+                const uint32_t ka = sm_a + L::stage_off + s * L::stage_bytes + L::q_bytes, vt = sm_a + L::vt_off + pb * L::vt_bytes;
+#pragma unroll
+                for (int ks = 0; ks < C / 16; ++ks)
+                    mma_bf16_ss(tb + L::tm_u + ob * 32, smem_desc(ka + 2 * ks * 1024, L::half_bytes, 1024, kSwz128),
+                                smem_desc(vt + 2 * ks * 128, 128, SBO_V, kSwzNone), idU, ks > 0);
+                mma_commit(&bars[BI.u_full + ob]);
+                mma_commit(&bars[BI.a_empty + pb]);
+                mma_commit(&bars[BI.empty + s]);
+            }
+        }
+    } else if (warp == 21) {
+        // ================= issuer: O2 = A_hi V + A_lo V (B operand = the V tile read MN-major, 32B swizzle) =================
+        if (lane == 0) {
+            constexpr uint32_t idO2 = idesc_bf16(C, kTcDVT, 0, 1);
+            for (uint32_t c = 0; c < n_chunks; ++c) {
+                const uint32_t s = c % NS, pb = c % NB, ob = c & 1;
+                mbar_wait(&bars[BI.full + s], (c / NS) & 1);
+                mbar_wait(&bars[BI.o_empty + ob], ((c >> 1) & 1) ^ 1);
+                mbar_wait(&bars[BI.a_full + pb], (c / NB) & 1);
+                tc_fence_after_sync();
+                TC_TRACE(4, c);
+                const uint32_t va = sm_a + L::stage_off + s * L::stage_bytes + 2 * L::q_bytes, aa = sm_a + L::a_off + pb * 2 * L::a_bytes;
+#pragma unroll
+                for (int term = 0; term < 2; ++term) {
+#pragma unroll
+                    for (int ks = 0; ks < C / 16; ++ks)
+                        mma_bf16_ss(tb + L::tm_o2 + ob * 16, smem_desc(aa + term * L::a_bytes + 2 * ks * 128, 128, SBO_A, kSwzNone),
+                                    smem_desc(va + 2 * ks * 256, 512, 256, kSwz32), idO2, (term | ks) > 0);
+                }
+                mma_commit(&bars[BI.o2_full + ob]);
+                mma_commit(&bars[BI.a_empty + pb]);
+                mma_commit(&bars[BI.empty + s]);
+            }
+        }
     }
     else if (warp >= 4 && warp < 12) {
         // ================= score warps: A = P ⊙ 2^(b_i - b_j) (causal), V~ = V ⊙ 2^(b_C - b_j) =================
@@ -365,10 +405,10 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             const float* b2 = gate + gslot * 2 * kGateBatch + (c % CPB) * C;
             mbar_wait(&bars[BI.full + s], (c / NS) & 1);
             mbar_wait(&bars[BI.a_empty + pb], ((c / NB) & 1) ^ 1);
-            if (q == 3 && lane == 0) TC_TRACE(10, c);
-            {   // V~ hi/lo, UMMA B operand MN-major interleaved: (n,k=token) -> (n/8)*SBO_V + (k/8)*128 + (k%8)*16 + (n%8)*2
+            if (q == 3 && lane == 0) TC_TRACE(5, c);
+            {   // [V~_hi | V~_lo], UMMA B operand MN-major interleaved: (n,k=token) -> (n/8)*SBO_V + (k/8)*128 + (k%8)*16 + (n%8)*2
                 const uint8_t* vs = sm + L::stage_off + s * L::stage_bytes + 2 * L::q_bytes;
-                uint8_t* vt = sm + L::vt_off + pb * 2 * L::vt_bytes;
+                uint8_t* vt = sm + L::vt_off + pb * L::vt_bytes;
                 const float b_last = b2[C - 1];
                 for (int idx = tid_s; idx < C * 2; idx += kSThreads) {
                     const int j = idx >> 1, half = idx & 1;
@@ -383,61 +423,64 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                     }
                     const uint32_t off = half * SBO_V + (j >> 3) * 128 + (j & 7) * 16;
                     *reinterpret_cast<uint4*>(vt + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-                    *reinterpret_cast<uint4*>(vt + L::vt_bytes + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+                    *reinterpret_cast<uint4*>(vt + 2 * SBO_V + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
                 }
             }
             mbar_wait(&bars[BI.p_full + pb], (c / NB) & 1);
             tc_fence_after_sync();
-            if (q == 3 && lane == 0) TC_TRACE(4, c);
             uint8_t* ah = sm + L::a_off + pb * 2 * L::a_bytes;
-            {
-                // 16-row group of this warp: row r of an M=64 tile sits in TMEM lane 32(r/16) + r%16, of an M=128 tile in lane r
-                const int rg = kAlt ? q : 2 * q + (int)wg;
-                const uint32_t lane_base = kAlt ? 32 * q : 32 * q + 16 * wg;
-                uint32_t r[C / 16][8];
+            // 16-row group of this warp: row r of an M=64 tile sits in TMEM lane 32(r/16) + r%16, of an M=128 tile in lane r
+            const int rg = kAlt ? q : 2 * q + (int)wg;
+            const uint32_t lane_base = kAlt ? 32 * q : 32 * q + 16 * wg;
+            const int ra = 16 * rg + (lane >> 2), rb = ra + 8;
+            const float ba = b2[ra], bb = b2[rb];
+            // UMMA A operand, K-major interleaved: (i,j) -> (i/8)*SBO_A + (j/8)*128 + (i%8)*16 + (j%8)*2
+            uint8_t* arow = ah + (ra >> 3) * SBO_A + (ra & 7) * 16 + (lane & 3) * 4;
 #pragma unroll
-                for (int cb = 0; cb < C / 16; ++cb)
-                    if (cb <= rg) tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_p + pb * C + cb * 16), r[cb]);
-                tmem_ld_wait();
-                tc_fence_before_sync();   // P(c) is in registers: the MMA thread may overwrite this TMEM buffer
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&bars[BI.p_empty + pb]);
-                if (q == 3 && lane == 0) TC_TRACE(11, c);
-                const int ra = 16 * rg + (lane >> 2), rb = ra + 8;
-                const float ba = b2[ra], bb = b2[rb];
-                // UMMA A operand, K-major interleaved: (i,j) -> (i/8)*SBO_A + (j/8)*128 + (i%8)*16 + (j%8)*2
-                uint8_t* arow = ah + (ra >> 3) * SBO_A + (ra & 7) * 16 + (lane & 3) * 4;
+            for (int cp = 0; cp < C / 32; ++cp) {   // two 16-column blocks per pass
+                if (2 * cp <= rg) {
+                    uint32_t r[2][8];
+                    tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_p + pb * C + (2 * cp) * 16), r[0]);
+                    if (2 * cp + 1 <= rg) tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_p + pb * C + (2 * cp + 1) * 16), r[1]);
+                    tmem_ld_wait();
+                    if (2 * cp + 2 > rg) {   // last pass of this warp: P(c) is in registers, the TMEM buffer may be overwritten
+                        tc_fence_before_sync();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&bars[BI.p_empty + pb]);
+                    }
 #pragma unroll
-                for (int cb = 0; cb < C / 16; ++cb) {
-                    if (cb <= rg) {
+                    for (int u = 0; u < 2; ++u) {
+                        const int cb = 2 * cp + u;
+                        if (cb <= rg) {
 #pragma unroll
-                        for (int jb = 0; jb < 2; ++jb) {
-                            const int j0 = cb * 16 + jb * 8 + 2 * (lane & 3);
-                            const float2 bj = *reinterpret_cast<const float2*>(b2 + j0);
-                            float a0 = __uint_as_float(r[cb][4 * jb + 0]) * ex2(ba - bj.x);
-                            float a1 = __uint_as_float(r[cb][4 * jb + 1]) * ex2(ba - bj.y);
-                            float c0 = __uint_as_float(r[cb][4 * jb + 2]) * ex2(bb - bj.x);
-                            float c1 = __uint_as_float(r[cb][4 * jb + 3]) * ex2(bb - bj.y);
-                            if (cb == rg) {   // diagonal block: causal mask j <= i
-                                a0 = (j0 <= ra) ? a0 : 0.f;
-                                a1 = (j0 + 1 <= ra) ? a1 : 0.f;
-                                c0 = (j0 <= rb) ? c0 : 0.f;
-                                c1 = (j0 + 1 <= rb) ? c1 : 0.f;
+                            for (int jb = 0; jb < 2; ++jb) {
+                                const int j0 = cb * 16 + jb * 8 + 2 * (lane & 3);
+                                const float2 bj = *reinterpret_cast<const float2*>(b2 + j0);
+                                float a0 = __uint_as_float(r[u][4 * jb + 0]) * ex2(ba - bj.x);
+                                float a1 = __uint_as_float(r[u][4 * jb + 1]) * ex2(ba - bj.y);
+                                float c0 = __uint_as_float(r[u][4 * jb + 2]) * ex2(bb - bj.x);
+                                float c1 = __uint_as_float(r[u][4 * jb + 3]) * ex2(bb - bj.y);
+                                if (cb == rg) {   // diagonal block: causal mask j <= i
+                                    a0 = (j0 <= ra) ? a0 : 0.f;
+                                    a1 = (j0 + 1 <= ra) ? a1 : 0.f;
+                                    c0 = (j0 <= rb) ? c0 : 0.f;
+                                    c1 = (j0 + 1 <= rb) ? c1 : 0.f;
+                                }
+                                uint32_t lo_a, lo_c;
+                                const uint32_t hi_a = split2(a0, a1, lo_a), hi_c = split2(c0, c1, lo_c);
+                                uint8_t* pa = arow + (cb * 2 + jb) * 128;
+                                *reinterpret_cast<uint32_t*>(pa) = hi_a;
+                                *reinterpret_cast<uint32_t*>(pa + L::a_bytes) = lo_a;
+                                *reinterpret_cast<uint32_t*>(pa + SBO_A) = hi_c;              // row + 8
+                                *reinterpret_cast<uint32_t*>(pa + SBO_A + L::a_bytes) = lo_c;
                             }
-                            uint32_t lo_a, lo_c;
-                            const uint32_t hi_a = split2(a0, a1, lo_a), hi_c = split2(c0, c1, lo_c);
-                            uint8_t* pa = arow + (cb * 2 + jb) * 128;
-                            *reinterpret_cast<uint32_t*>(pa) = hi_a;
-                            *reinterpret_cast<uint32_t*>(pa + L::a_bytes) = lo_a;
-                            *reinterpret_cast<uint32_t*>(pa + SBO_A) = hi_c;              // row + 8
-                            *reinterpret_cast<uint32_t*>(pa + SBO_A + L::a_bytes) = lo_c;
                         }
                     }
                 }
             }
             fence_proxy_async_smem();   // generic-proxy writes of A, V~ -> visible to tcgen05.mma's operand reads
             __syncwarp();
-            if (q == 3 && lane == 0) TC_TRACE(5, c);
+            if (q == 3 && lane == 0) TC_TRACE(6, c);
             if (lane == 0) {
                 mbar_arrive(&bars[BI.a_full + pb]);
                 mbar_arrive(&bars[BI.empty + s]);
@@ -446,26 +489,25 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 if (last_in_batch) mbar_arrive(&bars[BI.g_empty + gslot]);
             }
         }
-    } else if (warp >= 12) {
-        // ================= state warps: carry S, emit o =================
-        constexpr int NG = C / 64;
+    } else if (st_warp) {
+        // ================= state warps: the carry  S <- 2^(b_C) S + (Uh + Ul), fp32 FMA in registers =================
         for (uint32_t c = 0; c < n_chunks; ++c) {
             const uint32_t ob = c & 1, bt = c / CPB, gslot = bt & 1;
             mbar_wait(&bars[BI.g_full + gslot], (bt >> 1) & 1);
-            const float* eb = gate + gslot * 2 * kGateBatch + kGateBatch + (c % CPB) * C;
-            // ---- the carry: S <- 2^(b_C) S + U, fp32 FMA in registers ----
+            const float gam = gate[gslot * 2 * kGateBatch + kGateBatch + (c % CPB) * C + C - 1];
             mbar_wait(&bars[BI.u_full + ob], (c >> 1) & 1);
             tc_fence_after_sync();
-            if (q == 3 && lane == 0) TC_TRACE(6, c);
-            uint32_t ur[16];
-            tmem_ld_32x32b_x16(tmem_addr(tb, 32 * q, L::tm_u + ob * 16), ur);
+            uint32_t ur[32];
+            tmem_ld_32x32b_x32(tmem_addr(tb, 32 * q, L::tm_u + ob * 32), ur);
             tmem_ld_wait();
             tc_fence_before_sync();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&bars[BI.u_empty + ob]);
-            const float gam = eb[C - 1];
+            if (lane == 0) {
+                mbar_arrive(&bars[BI.u_empty + ob]);
+                if ((c % CPB) == CPB - 1 || c + 1 == n_chunks) mbar_arrive(&bars[BI.g_empty + gslot]);
+            }
 #pragma unroll
-            for (int j = 0; j < 16; ++j) S[j] = fmaf(gam, S[j], __uint_as_float(ur[j]));
+            for (int j = 0; j < 16; ++j) S[j] = fmaf(gam, S[j], __uint_as_float(ur[j]) + __uint_as_float(ur[16 + j]));
             if (c + 1 < n_chunks) {   // version c+1 of the S operand (read by O1(c+1))
                 const uint32_t sb = (c + 1) % NSB;
                 mbar_wait(&bars[BI.s_empty + sb], ((((c + 1) / NSB) & 1) ^ 1));
@@ -475,54 +517,62 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 if (lane == 0) mbar_arrive(&bars[BI.s_full + sb]);
             }
             if (q == 3 && lane == 0) TC_TRACE(7, c);
-            // ---- epilogue: o_i = 2^(b_i) O1_i + O2_i ----
-            mbar_wait(&bars[BI.o_full + ob], (c >> 1) & 1);
-            tc_fence_after_sync();
-            if (q == 3 && lane == 0) TC_TRACE(8, c);
-            const uint64_t t0 = (uint64_t)c * C;
-            const int n = (int)((T - t0) < (uint64_t)C ? (T - t0) : (uint64_t)C);
-#pragma unroll
-            for (int gi = 0; gi < NG; ++gi) {
-                const int rg = (C == 64) ? q : 2 * q + gi;
-                const uint32_t lane_base = (C == 64) ? 32 * q : 32 * q + 16 * gi;
-                uint32_t r1[8], r2[8];
-                tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_o1 + ob * 16), r1);
-                tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_o2 + ob * 16), r2);
-                tmem_ld_wait();
-                if (gi == NG - 1) {
-                    tc_fence_before_sync();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(&bars[BI.o_empty + ob]);
-                }
-                const int ra = 16 * rg + (lane >> 2), rb = ra + 8;
-                const float ea = eb[ra], ebb = eb[rb];
-                OutT* oa = o + (((size_t)b * t_stride + t0 + ra) * H + h) * DV + dv0 + 2 * (lane & 3);
-                OutT* oc = o + (((size_t)b * t_stride + t0 + rb) * H + h) * DV + dv0 + 2 * (lane & 3);
-#pragma unroll
-                for (int jb = 0; jb < 2; ++jb) {
-                    if (ra < n)
-                        store_o2<OutT>(oa + jb * 8, fmaf(ea, __uint_as_float(r1[4 * jb + 0]), __uint_as_float(r2[4 * jb + 0])),
-                                       fmaf(ea, __uint_as_float(r1[4 * jb + 1]), __uint_as_float(r2[4 * jb + 1])));
-                    if (rb < n)
-                        store_o2<OutT>(oc + jb * 8, fmaf(ebb, __uint_as_float(r1[4 * jb + 2]), __uint_as_float(r2[4 * jb + 2])),
-                                       fmaf(ebb, __uint_as_float(r1[4 * jb + 3]), __uint_as_float(r2[4 * jb + 3])));
-                }
-            }
-            __syncwarp();
-            if (q == 3 && lane == 0) TC_TRACE(9, c);
-            if (lane == 0 && ((c % CPB) == CPB - 1 || c + 1 == n_chunks)) mbar_arrive(&bars[BI.g_empty + gslot]);
         }
         if (st_active) {
             float4* p = reinterpret_cast<float4*>(state_out + ((size_t)bh * DK + krow) * DV + dv0);
 #pragma unroll
             for (int j = 0; j < 4; ++j) p[j] = make_float4(S[4 * j], S[4 * j + 1], S[4 * j + 2], S[4 * j + 3]);
         }
+    } else if (warp >= 16 && warp < 20) {
+        // ================= epilogue warps: o_i = 2^(b_i) (O1h_i + O1l_i) + O2_i =================
+        constexpr int NG = C / 64;
+        for (uint32_t c = 0; c < n_chunks; ++c) {
+            const uint32_t ob = c & 1, bt = c / CPB, gslot = bt & 1;
+            mbar_wait(&bars[BI.g_full + gslot], (bt >> 1) & 1);
+            const float* eb = gate + gslot * 2 * kGateBatch + kGateBatch + (c % CPB) * C;
+            mbar_wait(&bars[BI.o2_full + ob], (c >> 1) & 1);
+            mbar_wait(&bars[BI.o1_full + ob], (c >> 1) & 1);
+            tc_fence_after_sync();
+            const uint64_t t0 = (uint64_t)c * C;
+            const int n = (int)((T - t0) < (uint64_t)C ? (T - t0) : (uint64_t)C);
+#pragma unroll
+            for (int gi = 0; gi < NG; ++gi) {
+                const int rg = (C == 64) ? q : 2 * q + gi;
+                const uint32_t lane_base = (C == 64) ? 32 * q : 32 * q + 16 * gi;
+                uint32_t r1[16], r2[8];
+                tmem_ld_16x256b_x4(tmem_addr(tb, lane_base, L::tm_o1 + ob * 32), r1);
+                tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_o2 + ob * 16), r2);
+                tmem_ld_wait();
+                const int ra = 16 * rg + (lane >> 2), rb = ra + 8;
+                const float ea = eb[ra], ebb = eb[rb];
+                if (gi == NG - 1) {
+                    tc_fence_before_sync();
+                    __syncwarp();
+                    if (lane == 0) {
+                        mbar_arrive(&bars[BI.o_empty + ob]);
+                        if ((c % CPB) == CPB - 1 || c + 1 == n_chunks) mbar_arrive(&bars[BI.g_empty + gslot]);
+                    }
+                }
+                OutT* oa = o + (((size_t)b * t_stride + t0 + ra) * H + h) * DV + dv0 + 2 * (lane & 3);
+                OutT* oc = o + (((size_t)b * t_stride + t0 + rb) * H + h) * DV + dv0 + 2 * (lane & 3);
+#pragma unroll
+                for (int jb = 0; jb < 2; ++jb) {   // columns 8 jb + 2(t%4) + {0,1}: hi terms in block jb, lo terms in block 2 + jb
+                    const float h0 = __uint_as_float(r1[4 * jb + 0]) + __uint_as_float(r1[4 * (2 + jb) + 0]);
+                    const float h1 = __uint_as_float(r1[4 * jb + 1]) + __uint_as_float(r1[4 * (2 + jb) + 1]);
+                    const float h2 = __uint_as_float(r1[4 * jb + 2]) + __uint_as_float(r1[4 * (2 + jb) + 2]);
+                    const float h3 = __uint_as_float(r1[4 * jb + 3]) + __uint_as_float(r1[4 * (2 + jb) + 3]);
+                    if (ra < n) store_o2<OutT>(oa + jb * 8, fmaf(ea, h0, __uint_as_float(r2[4 * jb + 0])), fmaf(ea, h1, __uint_as_float(r2[4 * jb + 1])));
+                    if (rb < n) store_o2<OutT>(oc + jb * 8, fmaf(ebb, h2, __uint_as_float(r2[4 * jb + 2])), fmaf(ebb, h3, __uint_as_float(r2[4 * jb + 3])));
+                }
+            }
+            if (q == 3 && lane == 0) TC_TRACE(8, c);
+        }
     }
 
-    // ---- teardown: every tcgen05 op has completed (the state warps waited on the last commits) ----
+    // ---- teardown: every tcgen05 op has completed (the state and epilogue warps waited on the last commits) ----
     tc_fence_before_sync();
     __syncthreads();
-    if (warp == 1) tmem_dealloc(tb, L::tmem_cols);
+    if (warp == 2) tmem_dealloc(tb, L::tmem_cols);
 }
 
 // ---- host ---------------------------------------------------------------------------------------
