@@ -9,7 +9,7 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libesc.so")
+LIB_PATH = os.environ.get("ESC_LIB") or os.path.join(_HERE, "libesc.so")   # ESC_LIB: another build of the same ABI
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(
