@@ -26,8 +26,8 @@ inline int cuda_fail(cudaError_t e) {
 // One entry per (row, segment): `bytes` valid bytes from src to dst[0..n_dst).
 // Tiles of kCopyTileBytes are numbered globally; tile_begin[i] is the first tile of entry i.
 constexpr uint32_t kCopyThreads = 256;
-constexpr uint32_t kCopyUnroll = 4;                    // 16-byte vectors in flight per thread
-constexpr uint32_t kCopyTileBytes = kCopyThreads * kCopyUnroll * 16u;   // 16 KiB
+constexpr uint32_t kCopyUnroll = 2;                    // 16-byte vectors in flight per thread
+constexpr uint32_t kCopyTileBytes = kCopyThreads * kCopyUnroll * 16u;   // 8 KiB
 constexpr uint32_t kCopyMaxSeg = 112;                 // entries per launch (table <= 4 KiB kernel params)
 constexpr uint32_t kCopyMaxSegFork = 96;              // entries per fork launch
 
@@ -95,7 +95,7 @@ void layout_walk(const std::vector<Row>& rows, uint64_t P, std::vector<Seg>* seg
                  uint64_t* payload_bytes);
 
 // copy kernel launchers (copy_kernel.cu)
-int copy_grid_blocks(const esc_ctx* ctx);
+uint32_t copy_grid_blocks(uint64_t n_tiles);
 // Launch the copy of `n` (src,dst,bytes) entries, splitting into several launches only when n > kCopyMaxSeg.
 int launch_copy(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* dst, const uint64_t* bytes, uint32_t n,
                 cudaStream_t stream);

@@ -48,8 +48,7 @@ int esc_graph_capture(esc_ctx* ctx, esc_bufset* live, uint64_t max_boundary, con
         if (segs.size() > kCopyMaxSeg) return ESC_ERR_UNSUPPORTED;
         uint64_t tiles = 0;
         for (const Seg& s : segs) tiles += (s.bytes + kCopyTileBytes - 1) / kCopyTileBytes;
-        const uint64_t cap = (uint64_t)copy_grid_blocks(ctx);
-        grid = (uint32_t)(tiles < cap ? (tiles ? tiles : 1) : cap);
+        grid = copy_grid_blocks(tiles);   // one CTA per tile at max_boundary; CTAs beyond the bound capsule's tiles exit
     }
     // validate the scan layers and set kernel attributes BEFORE the capture begins
     std::vector<ScanShape> shapes(n_layers);
