@@ -3,7 +3,7 @@
 // Definition (BASELINE.json north_star; "a fold over the entire prefix", folded "per
 // chunk" PAPER.md:169):   S_t = g_t S_{t-1} + k_t^T v_t ,  o_t = q_t S_t.
 // Chunk algebra (exact-arithmetic equivalent; every exponent <= 0), with b_i = sum_{r<=i} log2 g_r:
-//     P      = Q K^T                                  (C x C)     tcgen05.mma  M=C   N=C   K=d_k
+//     P      = Q K^T                                  (C x C)     tcgen05.mma  M=C   N=C/CS  K=d_k  (a column slice per CTA)
 //     A_ij   = P_ij 2^(b_i - b_j) [j <= i]            fp32 ALU + MUFU, split into bf16 hi + lo
 //     O1     = Q [S_hi | S_lo]                        (C x 32)    tcgen05.mma  M=C   N=32  K=d_k
 //     O2     = A_hi V + A_lo V                        (C x 16)    tcgen05.mma  M=C   N=16  K=C  (x2)
@@ -11,23 +11,40 @@
 //     U      = K^T [V~_hi | V~_lo] , V~_j = 2^(b_C - b_j) v_j   (d_k x 32)  tcgen05.mma  M=d_k N=32 K=C
 //     S_next = 2^(b_C) S_prev + (Uh + Ul)             fp32 FMA in registers (the carry chain)
 //
-// One CTA owns (b, h, 16 columns of d_v) — the columns of S are independent — and walks the chunks
-// in order.  Only the last line is a true dependency between chunks, and only O1 reads the carried
-// state, so the kernel is a software pipeline of specialised warps synchronised by mbarriers only:
-//   warp 0       TMA producer: Q / K / V chunk tiles -> 128B/32B-swizzled smem ring (+ L2 prefetch ahead)
-//   warp 1       gate warp: log2 g, segmented warp-shuffle prefix sums, 256 tokens per batch
-//   warps 2,3,20,21  MMA issuers, one thread each: P | O1 | U | O2.  A tcgen05.mma costs its issuing
-//                thread ~55 cycles whatever its shape (measured), the tensor pipe only max(23, M'N/256):
-//                four issuers keep the pipe, not the issue slot, the limit, and give every product its
-//                own dependency chain (no head-of-line blocking behind the state-dependent O1)
-//   warps 4-11   score warps (2 groups): P (TMEM) -> A hi/lo (smem, UMMA K-major interleaved), V -> V~
-//   warps 12-15  state warps: U (TMEM) -> carry S in fp32 registers -> [S_hi | S_lo] operand
-//   warps 16-19  epilogue warps: O1, O2 (TMEM) -> o (global)
+// Decomposition.  The columns of S are independent, so one CTA owns (b, h, 16 columns of d_v) and walks
+// the chunks in order with its state slice in registers.  CS = 4 neighbouring d_v slices of a head form a
+// THREAD-BLOCK CLUSTER and share everything that does not depend on the d_v slice:
+//   * Q and K tiles: CTA r loads rows [r C/CS, (r+1) C/CS) of each tile and TMA-multicasts them into the
+//     same stage of all CS CTAs (L2 -> SM traffic for Q, K drops CS-fold);
+//   * the scores: CTA r computes only the column slice P[:, r C/CS ...] (an N = C/CS MMA), turns it into
+//     the A slice (decay, causal mask, hi/lo split) in its own A operand buffer and pushes that contiguous
+//     slice into the same place of every peer's buffer with one bulk shared::cta -> shared::cluster copy
+//     per peer, completing (tx bytes) on the peer's mbarrier.
+// Ring and A-buffer reuse are therefore cluster-wide events: stage / A-buffer "empty" barriers count
+// tcgen05.commit arrivals multicast from all CS CTAs.  The score path (P -> A -> O2) has its own buffers
+// (NB of each, O2 reads V from a copy the V~ warps make), so it never holds an input stage.
+// What bounds it (r01, ncu + clock64 traces): shared-memory bandwidth.  Per chunk a CTA moves ~160 KB
+// through its shared memory (34 KB TMA writes, 84 KB tcgen05.mma operand reads — Q twice, K, A, each for
+// a 16..32-column B operand — 24 KB of A-slice exchange, 16 KB of V~ / S operand writes) = ~1270 cycles at
+// 128 B/clk against a measured period of ~1400; ALU, MUFU, issue-slot and spin-wait ablations moved
+// nothing.  The d_v split that fills the SMs at B H = 16 is what makes the A operands (Q, K, A) be
+// re-read per 16 output columns.
+//
+// Warp roles (22 warps, mbarrier-synchronised software pipeline, no CTA-wide barrier in the loop):
+//   warp 0         TMA producer (multicast Q/K row slices, own V slice; L2 prefetch ahead)
+//   warp 1         gate warp: log2 g, segmented warp-shuffle prefix sums, 256 tokens per batch
+//   warps 2,3,4,5  MMA issuers, one thread each: P | O1 | U | O2 (a tcgen05.mma costs its issuing thread
+//                  ~55 cycles whatever its shape: four issuers keep the pipe, not the issue slot, the limit)
+//   warps 6,7,20,21  V~ warps: V -> V~ hi/lo operand (own barrier: U and the carry never wait for scores)
+//   warps 8-11     score warps (one per TMEM lane quadrant): P slice (TMEM) -> A slice -> all CTAs
+//   warps 12-15    state warps: U (TMEM) -> carry S in fp32 registers -> [S_hi | S_lo] operand
+//   warps 16-19    epilogue warps: O1, O2 (TMEM) -> o (global)
 //
 // Bit-identity: the carry is a pure function of (S_prev bits, chunk inputs); there
 // is no T-dependent tiling, no atomics, no split-K; every accumulator is produced by ONE issuer thread
-// in a fixed order.  Precision: raw Q, K, V are the bf16 inputs; A, V~, S_prev are
-// two-term bf16 splits (hi + lo), the hi|lo halves of V~ and S ride in one MMA as 32 columns.
+// in a fixed order, every A element by one thread of one CTA.  Precision: raw Q, K, V
+// are the bf16 inputs; A, V~, S_prev are two-term bf16 splits (hi + lo), the hi|lo halves of V~ and S
+// ride in one MMA as 32 columns.
 #include <cuda.h>
 #include <cuda_bf16.h>
 
@@ -45,6 +62,7 @@ constexpr int kTcDVT = 16;        // d_v columns per CTA
 constexpr int kTcNM = 2 * kTcDVT; // columns of a merged hi|lo operand
 constexpr int kGateBatch = 256;   // tokens per gate-warp batch
 constexpr int kPrefetchAhead = 6; // chunks the producer prefetches into L2 ahead of its smem ring
+constexpr int kVtThreads = 128;   // threads of the four V~ warps
 
 #ifdef ESC_TC_TRACE   // bring-up only: per-chunk clock64() stamps of CTA (0,0), read back with esc_debug_trace_read
 __device__ long long g_tc_trace[16 * 64];
@@ -56,41 +74,46 @@ __device__ long long g_tc_trace[16 * 64];
 template <int DK, int C>
 struct TcCfg {
     static constexpr int NS = (C == 64) ? 4 : 2;          // input stages
-    static constexpr int NB = (C == 64) ? 2 : 1;          // P / A / V~ buffers
+    static constexpr int NB = (C == 64) ? 3 : 1;          // P / A / V~ (+ V copy) buffers
     static constexpr int NSB = (C == 64) ? 2 : 1;         // S operand buffers
-    static constexpr int SWA = (C == 64) ? 4 : 8;         // score-warp arrivals per chunk (one / both score groups)
     static constexpr int NH = DK / 64;                    // 64-column halves of a Q / K tile
     static constexpr int CPB = kGateBatch / C;            // chunks per gate batch
     static constexpr uint32_t half_bytes = C * 128;       // one [C x 64] bf16 half tile
     static constexpr uint32_t q_bytes = NH * half_bytes;
     static constexpr uint32_t v_bytes = C * 32;           // [C x 16] bf16
     static constexpr uint32_t stage_bytes = 2 * q_bytes + v_bytes;   // multiple of 1024
-    static constexpr uint32_t a_bytes = C * C * 2;        // one A term
-    static constexpr uint32_t vt_bytes = C * kTcNM * 2;   // merged V~ operand [32 x C]
+    // A operand (M = C rows i, K = C keys j), K-major, no swizzle, hi and lo terms interleaved per 8-key group:
+    //   (term, i, j) -> (j/8) a_lbo + term a_term + (i/8) 128 + (i%8) 16 + (j%8) 2
+    // so that the 8-key groups of one CTA's column slice are contiguous (one bulk copy per 16-row group and term)
+    static constexpr uint32_t a_term = (C / 8) * 128;     // one term of one 8-key group: [C x 8] bf16
+    static constexpr uint32_t a_lbo = 2 * a_term;
+    static constexpr uint32_t a_bytes = (C / 8) * a_lbo;  // both terms
+    static constexpr uint32_t vc_off = C * kTcNM * 2;     // V~ buffer: merged V~ operand [32 x C], then a copy of the V tile
+    static constexpr uint32_t vt_bytes = vc_off + v_bytes;
     static constexpr uint32_t s_bytes = DK * kTcNM * 2;   // merged S operand [32 x DK]
     // offsets from the 1024-aligned base
     static constexpr uint32_t stage_off = 0;
-    static constexpr uint32_t a_off = stage_off + NS * stage_bytes;             // [NB][hi,lo]
-    static constexpr uint32_t vt_off = a_off + NB * 2 * a_bytes;                // [NB]
+    static constexpr uint32_t a_off = stage_off + NS * stage_bytes;             // [NB]
+    static constexpr uint32_t vt_off = a_off + NB * a_bytes;                    // [NB]
     static constexpr uint32_t s_off = vt_off + NB * vt_bytes;                   // [NSB]
     static constexpr uint32_t gate_off = s_off + NSB * s_bytes;                 // [2][b2[256], eb[256]] fp32
     static constexpr uint32_t bar_off = gate_off + 2 * 2 * kGateBatch * 4;
-    static constexpr uint32_t n_bars = 2 * NS + 4 * NB + 2 * NSB + 14;
+    static constexpr uint32_t n_bars = 2 * NS + 6 * NB + 2 * NSB + 14;
     static constexpr uint32_t total = bar_off + 64 * 8 + 16 + 1024;             // + alignment slack
-    static constexpr uint32_t tmem_cols = 512;
-    static constexpr uint32_t tm_p = 0;                    // [NB] x C columns
-    static constexpr uint32_t tm_u = NB * C;               // [2] x 32
-    static constexpr uint32_t tm_o1 = tm_u + 64;           // [2] x 32
-    static constexpr uint32_t tm_o2 = tm_o1 + 64;          // [2] x 16
-    static_assert(tm_o2 + 32 <= tmem_cols, "TMEM budget");
+    static constexpr uint32_t tmem_cols = 256;
+    static constexpr uint32_t tm_p = 0;                    // [NB] x 32 columns (a slice has C/CS <= 32)
+    static constexpr uint32_t tm_u = 96;                   // [2] x 32
+    static constexpr uint32_t tm_o1 = 160;                 // [2] x 32
+    static constexpr uint32_t tm_o2 = 224;                 // [2] x 16
+    static_assert(NB * 32 <= tm_u, "TMEM budget");
     static_assert(stage_bytes % 1024 == 0, "stages must keep 1024-byte alignment (128B swizzle)");
     static_assert(n_bars <= 64, "barrier area");
     static_assert(total <= 232448, "shared memory budget");
 };
 
 struct TcBars {   // indices into the mbarrier array
-    int full, empty, p_full, p_empty, a_full, a_empty, s_full, s_empty, o1_full, o2_full, o_empty, u_full, u_empty, g_full,
-        g_empty;
+    int full, empty, p_full, p_empty, a_full, a_empty, vt_full, vt_empty, s_full, s_empty, o1_full, o2_full, o_empty, u_full,
+        u_empty, g_full, g_empty;
 };
 template <int DK, int C>
 __device__ __forceinline__ constexpr TcBars tc_bars() {
@@ -103,6 +126,8 @@ __device__ __forceinline__ constexpr TcBars tc_bars() {
     b.p_empty = i; i += L::NB;
     b.a_full = i; i += L::NB;
     b.a_empty = i; i += L::NB;
+    b.vt_full = i; i += L::NB;
+    b.vt_empty = i; i += L::NB;
     b.s_full = i; i += L::NSB;
     b.s_empty = i; i += L::NSB;
     b.o1_full = i; i += 2;
@@ -142,34 +167,80 @@ __device__ __forceinline__ void store_o2<bf16>(bf16* p, float x0, float x1) {
     *reinterpret_cast<uint32_t*>(p) = pack_bf16(x0, x1);
 }
 
-template <int DK, int C, typename OutT>
+// 16 TMEM lanes x NA fp32 columns -> NA/2 registers per thread (layout: see tmem_ld_16x256b_x2 in sm100_ptx.cuh)
+template <int NA>
+__device__ __forceinline__ void tmem_ld_slice(uint32_t addr, uint32_t* r) {
+    if constexpr (NA == 8) tmem_ld_16x256b_x1(addr, r);
+    else if constexpr (NA == 16) tmem_ld_16x256b_x2(addr, r);
+    else tmem_ld_16x256b_x4(addr, r);
+}
+
+template <int DK, int C, int CS, typename OutT>
 __global__ void __launch_bounds__(kTcThreads, 1)
 esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tk,
                    const __grid_constant__ CUtensorMap tv, const float* __restrict__ g, const float* state_in,
                    float* state_out, OutT* __restrict__ o, uint32_t H, uint32_t DV, uint64_t T, uint64_t t_stride) {
     using L = TcCfg<DK, C>;
     constexpr TcBars BI = tc_bars<DK, C>();
-    constexpr int NS = L::NS, NB = L::NB, NSB = L::NSB, SWA = L::SWA, CPB = L::CPB;
-    constexpr uint32_t SBO_A = (C / 8) * 128, SBO_V = (C / 8) * 128, SBO_S = (DK / 8) * 128;
+    constexpr int NS = L::NS, NB = L::NB, NSB = L::NSB, CPB = L::CPB;
+    constexpr int NA = C / CS;                      // keys per score slice = Q / K rows this CTA loads
+    constexpr uint16_t kAll = (uint16_t)((1u << CS) - 1);
+    constexpr uint32_t SBO_V = (C / 8) * 128, SBO_S = (DK / 8) * 128;
+    static_assert(NA == 8 || NA == 16 || NA == 32, "slice width");
+    static_assert(C == 128 ? NA >= 16 : true, "an M = 128 MMA needs N % 16 == 0");
 
     extern __shared__ uint8_t smem_raw[];
-    uint8_t* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint8_t* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // same offset in every CTA of the cluster
     const uint32_t sm_a = smem_u32(sm);
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + L::bar_off);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sm + L::bar_off + 64 * 8);
     float* gate = reinterpret_cast<float*>(sm + L::gate_off);   // [2][2][256]: b2 then eb per slot
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();   // clusters are CS consecutive d_v slices (blockIdx.x) of one (b, h)
     const uint32_t bh = blockIdx.y, b = bh / H, h = bh % H, dv0 = blockIdx.x * kTcDVT;
+    const uint32_t key0 = rank * NA;    // first key (= first Q / K row) of this CTA's slice
     const uint32_t n_chunks = (uint32_t)((T + C - 1) / C);
     const int q = warp & 3;   // TMEM lane quadrant this warp may access
+    if (threadIdx.x == 0) TC_TRACE(9, 0);
+    // Programmatic dependent launch: the next kernel of the stream / graph (typically the next layer's scan) may start
+    // its on-chip setup while this one runs; everything this kernel reads from or writes to global memory comes after
+    // griddepcontrol.wait below, i.e. after the preceding kernel has completed and flushed.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
-    // ---- one-time setup ----------------------------------------------------------------------------
+    // TMA producer steps (warp 0, lane 0)
+    auto tma_prefetch_chunk = [&](uint32_t c) {   // pull this CTA's share of chunk c into L2
+        const int t0 = (int)(c * C);
+#pragma unroll
+        for (int hh = 0; hh < L::NH; ++hh) {
+            tma_prefetch_4d(&tq, hh * 64, (int)h, t0 + (int)key0, (int)b);
+            tma_prefetch_4d(&tk, hh * 64, (int)h, t0 + (int)key0, (int)b);
+        }
+        tma_prefetch_4d(&tv, (int)dv0, (int)h, t0, (int)b);
+    };
+    auto tma_issue = [&](uint32_t c) {   // chunk c -> stage c % NS of ALL CTAs (Q, K rows key0..) / of this CTA (V)
+        const uint32_t s = c % NS;
+        uint8_t* st = sm + L::stage_off + s * L::stage_bytes;
+        uint64_t* full = &bars[BI.full + s];
+        mbar_arrive_expect_tx(full, L::stage_bytes);   // Q and K arrive in CS row slices, one from each CTA
+        const int t0 = (int)(c * C);
+#pragma unroll
+        for (int hh = 0; hh < L::NH; ++hh) {
+            tma_load_4d_mc(st + hh * L::half_bytes + key0 * 128, &tq, full, hh * 64, (int)h, t0 + (int)key0, (int)b, kAll);
+            tma_load_4d_mc(st + L::q_bytes + hh * L::half_bytes + key0 * 128, &tk, full, hh * 64, (int)h, t0 + (int)key0, (int)b,
+                           kAll);
+        }
+        tma_load_4d(st + 2 * L::q_bytes, &tv, full, (int)dv0, (int)h, t0, (int)b);
+        TC_TRACE(0, c);
+    };
+
+    // ---- one-time setup, on-chip part (under programmatic dependent launch it overlaps the preceding kernel) -----------
     if (warp == 0 && lane == 0) {
-        for (int i = 0; i < NS; ++i) { mbar_init(&bars[BI.full + i], 1); mbar_init(&bars[BI.empty + i], 4 + SWA); }
+        for (int i = 0; i < NS; ++i) { mbar_init(&bars[BI.full + i], 1); mbar_init(&bars[BI.empty + i], 3 * CS); }
         for (int i = 0; i < NB; ++i) {
-            mbar_init(&bars[BI.p_full + i], 1); mbar_init(&bars[BI.p_empty + i], SWA);
-            mbar_init(&bars[BI.a_full + i], SWA); mbar_init(&bars[BI.a_empty + i], 2);
+            mbar_init(&bars[BI.p_full + i], 1); mbar_init(&bars[BI.p_empty + i], 4);
+            mbar_init(&bars[BI.a_full + i], 4); mbar_init(&bars[BI.a_empty + i], CS);
+            mbar_init(&bars[BI.vt_full + i], 4); mbar_init(&bars[BI.vt_empty + i], 2);
         }
         for (int i = 0; i < NSB; ++i) { mbar_init(&bars[BI.s_full + i], 4); mbar_init(&bars[BI.s_empty + i], 1); }
         for (int i = 0; i < 2; ++i) {
@@ -181,9 +252,17 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
         tma_prefetch_desc(&tq); tma_prefetch_desc(&tk); tma_prefetch_desc(&tv);
     }
     if (warp == 2) tmem_alloc(tmem_slot, L::tmem_cols);
-    // A buffers: the strictly-upper 16x16 blocks are never written again and must read as zero
-    for (uint32_t i = threadIdx.x; i < NB * 2 * L::a_bytes / 16; i += kTcThreads)
+    // A buffers: blocks above the causal diagonal are never written by any CTA and must read as zero
+    for (uint32_t i = threadIdx.x; i < NB * L::a_bytes / 16; i += kTcThreads)
         reinterpret_cast<uint4*>(sm + L::a_off)[i] = make_uint4(0, 0, 0, 0);
+    fence_proxy_async_smem();
+    tc_fence_before_sync();
+    // every CTA's barriers are initialised and its A buffers zeroed before any peer multicasts / copies into them
+    cluster_sync();
+    tc_fence_after_sync();
+    const uint32_t tb = *tmem_slot;
+    asm volatile("griddepcontrol.wait;" ::: "memory");   // ---- global memory may be touched from here on ----
+    if (threadIdx.x == 0) TC_TRACE(10, 0);
 
     // state warps own the carry: row `krow` of the [d_k x 16] slice per thread, fp32 registers
     const bool st_warp = warp >= 12 && warp < 16;
@@ -207,57 +286,21 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             }
         }
     };
-    if (st_warp) {
-#pragma unroll
-        for (int j = 0; j < 16; ++j) S[j] = 0.f;
-        if (st_active && state_in) {
-            const float4* p = reinterpret_cast<const float4*>(state_in + ((size_t)bh * DK + krow) * DV + dv0);
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const float4 x = p[j];
-                S[4 * j] = x.x; S[4 * j + 1] = x.y; S[4 * j + 2] = x.z; S[4 * j + 3] = x.w;
-            }
-        }
-        write_s_operand(0);
-    }
-    fence_proxy_async_smem();
-    tc_fence_before_sync();
-    __syncthreads();
-    tc_fence_after_sync();
-    const uint32_t tb = *tmem_slot;
-    if (st_warp && lane == 0) mbar_arrive(&bars[BI.s_full]);   // version 0 of the S operand is in place
 
     if (warp == 0) {
         // ================= TMA producer =================
         if (lane == 0) {
-            auto prefetch = [&](uint32_t c) {   // pull chunk c's tiles into L2 (Q, K once per head: by the dv-slice-0 CTA)
-                const int t0 = (int)(c * C);
-                if (blockIdx.x == 0) {
-#pragma unroll
-                    for (int hh = 0; hh < L::NH; ++hh) {
-                        tma_prefetch_4d(&tq, hh * 64, (int)h, t0, (int)b);
-                        tma_prefetch_4d(&tk, hh * 64, (int)h, t0, (int)b);
-                    }
-                }
-                tma_prefetch_4d(&tv, (int)dv0, (int)h, t0, (int)b);
-            };
-            for (uint32_t c = NS; c < n_chunks && c < NS + kPrefetchAhead; ++c) prefetch(c);
+            for (uint32_t c = NS; c < n_chunks && c < (uint32_t)(NS + kPrefetchAhead); ++c) tma_prefetch_chunk(c);
             for (uint32_t c = 0; c < n_chunks; ++c) {
-                const uint32_t s = c % NS;
-                if (c + NS + kPrefetchAhead < n_chunks) prefetch(c + NS + kPrefetchAhead);
-                mbar_wait(&bars[BI.empty + s], ((c / NS) & 1) ^ 1);
-                uint8_t* st = sm + L::stage_off + s * L::stage_bytes;
-                uint64_t* full = &bars[BI.full + s];
-                mbar_arrive_expect_tx(full, L::stage_bytes);
-                const int t0 = (int)(c * C);
-#pragma unroll
-                for (int hh = 0; hh < L::NH; ++hh) {
-                    tma_load_4d(st + hh * L::half_bytes, &tq, full, hh * 64, (int)h, t0, (int)b);
-                    tma_load_4d(st + L::q_bytes + hh * L::half_bytes, &tk, full, hh * 64, (int)h, t0, (int)b);
-                }
-                tma_load_4d(st + 2 * L::q_bytes, &tv, full, (int)dv0, (int)h, t0, (int)b);
-                TC_TRACE(0, c);
+                if (c + NS + kPrefetchAhead < n_chunks) tma_prefetch_chunk(c + NS + kPrefetchAhead);
+                // the stage is free once the P, O1 and U issuers of all CS CTAs have committed chunk c - NS (this CTA writes into all
+                // of them); O2 reads V from the copy the V~ warps made, so the score path never holds a stage
+                mbar_wait_relaxed(&bars[BI.empty + c % NS], ((c / NS) & 1) ^ 1);
+                tma_issue(c);
             }
+            // tail: every peer's last commits have reached this CTA's barriers before anyone may exit
+            for (uint32_t c = n_chunks > (uint32_t)NS ? n_chunks - NS : 0; c < n_chunks; ++c)
+                mbar_wait(&bars[BI.empty + c % NS], (c / NS) & 1);
         }
     } else if (warp == 1) {
         // ================= gate warp: b2_i = sum_{r<=i in chunk} log2 g_r, 256 tokens per batch =================
@@ -289,7 +332,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             const float prev = __shfl_up_sync(0xffffffffu, incl, 1);
             const float excl = (lane % GL) ? prev : 0.f;
             const uint32_t slot = bt & 1;
-            mbar_wait(&bars[BI.g_empty + slot], ((bt >> 1) & 1) ^ 1);
+            mbar_wait_relaxed(&bars[BI.g_empty + slot], ((bt >> 1) & 1) ^ 1);
             float* b2 = gate + slot * 2 * kGateBatch;
             float* eb = b2 + kGateBatch;
 #pragma unroll
@@ -302,23 +345,23 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             if (lane == 0) mbar_arrive(&bars[BI.g_full + slot]);
         }
     } else if (warp == 2) {
-        // ================= issuer: P = Q K^T =================
+        // ================= issuer: P[:, key0 .. key0+NA) = Q K[key0 .. key0+NA)^T =================
         if (lane == 0) {
-            constexpr uint32_t idP = idesc_bf16(C, C, 0, 0);
+            constexpr uint32_t idP = idesc_bf16(C, NA, 0, 0);
             for (uint32_t c = 0; c < n_chunks; ++c) {
                 const uint32_t s = c % NS, pb = c % NB;
                 mbar_wait(&bars[BI.full + s], (c / NS) & 1);
                 mbar_wait(&bars[BI.p_empty + pb], ((c / NB) & 1) ^ 1);
                 tc_fence_after_sync();
-                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes, ka = qa + L::q_bytes;
+                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes, ka = qa + L::q_bytes + key0 * 128;
 #pragma unroll
                 for (int ks = 0; ks < DK / 16; ++ks) {
                     const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
-                    mma_bf16_ss(tb + L::tm_p + pb * C, smem_desc(qa + off, 16, 1024, kSwz128),
+                    mma_bf16_ss(tb + L::tm_p + pb * 32, smem_desc(qa + off, 16, 1024, kSwz128),
                                 smem_desc(ka + off, 16, 1024, kSwz128), idP, ks > 0);
                 }
                 mma_commit(&bars[BI.p_full + pb]);
-                mma_commit(&bars[BI.empty + s]);
+                mma_commit_mc(&bars[BI.empty + s], kAll);
                 TC_TRACE(1, c);
             }
         }
@@ -342,10 +385,10 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 }
                 mma_commit(&bars[BI.s_empty + sb]);
                 mma_commit(&bars[BI.o1_full + ob]);
-                mma_commit(&bars[BI.empty + s]);
+                mma_commit_mc(&bars[BI.empty + s], kAll);
             }
         }
-    } else if (warp == 20) {
+    } else if (warp == 4) {
         // ================= issuer: U = K^T [V~_hi | V~_lo] (A operand = the K tile read MN-major) =================
         if (lane == 0) {
             constexpr uint32_t idU = idesc_bf16(DK, kTcNM, 1, 1);
@@ -353,7 +396,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 const uint32_t s = c % NS, pb = c % NB, ob = c & 1;
                 mbar_wait(&bars[BI.full + s], (c / NS) & 1);
                 mbar_wait(&bars[BI.u_empty + ob], ((c >> 1) & 1) ^ 1);
-                mbar_wait(&bars[BI.a_full + pb], (c / NB) & 1);
+                mbar_wait(&bars[BI.vt_full + pb], (c / NB) & 1);   // the V~ warps are then also done with the stage's V tile
                 tc_fence_after_sync();
                 TC_TRACE(3, c);
                 const uint32_t ka = sm_a + L::stage_off + s * L::stage_bytes + L::q_bytes, vt = sm_a + L::vt_off + pb * L::vt_bytes;
@@ -362,135 +405,179 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                     mma_bf16_ss(tb + L::tm_u + ob * 32, smem_desc(ka + 2 * ks * 1024, L::half_bytes, 1024, kSwz128),
                                 smem_desc(vt + 2 * ks * 128, 128, SBO_V, kSwzNone), idU, ks > 0);
                 mma_commit(&bars[BI.u_full + ob]);
-                mma_commit(&bars[BI.a_empty + pb]);
-                mma_commit(&bars[BI.empty + s]);
+                mma_commit(&bars[BI.vt_empty + pb]);
+                mma_commit_mc(&bars[BI.empty + s], kAll);
             }
         }
-    } else if (warp == 21) {
-        // ================= issuer: O2 = A_hi V + A_lo V (B operand = the V tile read MN-major, 32B swizzle) =================
+    } else if (warp == 5) {
+        // ================= issuer: O2 = A_hi V + A_lo V (B operand = the V tile copy, MN-major, 32B swizzle) =================
         if (lane == 0) {
             constexpr uint32_t idO2 = idesc_bf16(C, kTcDVT, 0, 1);
             for (uint32_t c = 0; c < n_chunks; ++c) {
-                const uint32_t s = c % NS, pb = c % NB, ob = c & 1;
-                mbar_wait(&bars[BI.full + s], (c / NS) & 1);
+                const uint32_t pb = c % NB, ob = c & 1;
                 mbar_wait(&bars[BI.o_empty + ob], ((c >> 1) & 1) ^ 1);
-                mbar_wait(&bars[BI.a_full + pb], (c / NB) & 1);
+                mbar_wait(&bars[BI.vt_full + pb], (c / NB) & 1);   // the V copy
+                mbar_wait(&bars[BI.a_full + pb], (c / NB) & 1);    // own slice written + every peer's slice landed
                 tc_fence_after_sync();
                 TC_TRACE(4, c);
-                const uint32_t va = sm_a + L::stage_off + s * L::stage_bytes + 2 * L::q_bytes, aa = sm_a + L::a_off + pb * 2 * L::a_bytes;
+                const uint32_t va = sm_a + L::vt_off + pb * L::vt_bytes + L::vc_off, aa = sm_a + L::a_off + pb * L::a_bytes;
 #pragma unroll
                 for (int term = 0; term < 2; ++term) {
 #pragma unroll
                     for (int ks = 0; ks < C / 16; ++ks)
-                        mma_bf16_ss(tb + L::tm_o2 + ob * 16, smem_desc(aa + term * L::a_bytes + 2 * ks * 128, 128, SBO_A, kSwzNone),
+                        mma_bf16_ss(tb + L::tm_o2 + ob * 16, smem_desc(aa + term * L::a_term + 2 * ks * L::a_lbo, L::a_lbo, 128, kSwzNone),
                                     smem_desc(va + 2 * ks * 256, 512, 256, kSwz32), idO2, (term | ks) > 0);
                 }
                 mma_commit(&bars[BI.o2_full + ob]);
-                mma_commit(&bars[BI.a_empty + pb]);
-                mma_commit(&bars[BI.empty + s]);
+                mma_commit(&bars[BI.vt_empty + pb]);
+                mma_commit_mc(&bars[BI.a_empty + pb], kAll);   // every CTA writes into this buffer: all of them must know
             }
         }
-    }
-    else if (warp >= 4 && warp < 12) {
-        // ================= score warps: A = P ⊙ 2^(b_i - b_j) (causal), V~ = V ⊙ 2^(b_C - b_j) =================
-        // two groups of 4 warps (one warp per TMEM lane quadrant).  C = 64: the groups alternate chunks (and own the
-        // P / A / V~ buffer of their parity).  C = 128: both groups work on every chunk, one 16-row group per quadrant each.
-        const uint32_t wg = (uint32_t)(warp - 4) >> 2;
-        constexpr bool kAlt = (C == 64);
-        const int tid_s = kAlt ? ((warp - 4) & 3) * 32 + lane : (warp - 4) * 32 + lane;   // index among the threads sharing a chunk
-        constexpr int kSThreads = kAlt ? 128 : 256;
-        for (uint32_t c = kAlt ? wg : 0; c < n_chunks; c += kAlt ? 2 : 1) {
+    } else if (warp == 6 || warp == 7 || warp == 20 || warp == 21) {
+        // ================= V~ warps: [V~_hi | V~_lo], V~_j = 2^(b_C - b_j) v_j, and a copy of V for O2 =================
+        // UMMA B operand, MN-major interleaved: (n,k=token) -> (n/8)*SBO_V + (k/8)*128 + (k%8)*16 + (n%8)*2
+        const int tid_v = (warp < 8 ? warp - 6 : warp - 18) * 32 + lane;
+        for (uint32_t c = 0; c < n_chunks; ++c) {
             const uint32_t s = c % NS, pb = c % NB, bt = c / CPB, gslot = bt & 1;
             mbar_wait(&bars[BI.g_full + gslot], (bt >> 1) & 1);
             const float* b2 = gate + gslot * 2 * kGateBatch + (c % CPB) * C;
             mbar_wait(&bars[BI.full + s], (c / NS) & 1);
-            mbar_wait(&bars[BI.a_empty + pb], ((c / NB) & 1) ^ 1);
-            if (q == 3 && lane == 0) TC_TRACE(5, c);
-            {   // [V~_hi | V~_lo], UMMA B operand MN-major interleaved: (n,k=token) -> (n/8)*SBO_V + (k/8)*128 + (k%8)*16 + (n%8)*2
-                const uint8_t* vs = sm + L::stage_off + s * L::stage_bytes + 2 * L::q_bytes;
-                uint8_t* vt = sm + L::vt_off + pb * L::vt_bytes;
-                const float b_last = b2[C - 1];
-                for (int idx = tid_s; idx < C * 2; idx += kSThreads) {
-                    const int j = idx >> 1, half = idx & 1;
-                    const uint4 raw = *reinterpret_cast<const uint4*>(vs + j * 32 + ((half ^ ((j >> 2) & 1)) * 16));   // undo 32B swizzle
-                    const float sc = ex2(b_last - b2[j]);
-                    const uint32_t w[4] = {raw.x, raw.y, raw.z, raw.w};
-                    uint32_t hi[4], lo[4];
+            mbar_wait(&bars[BI.vt_empty + pb], ((c / NB) & 1) ^ 1);
+            const uint8_t* vs = sm + L::stage_off + s * L::stage_bytes + 2 * L::q_bytes;
+            uint8_t* vt = sm + L::vt_off + pb * L::vt_bytes;
+            const float b_last = b2[C - 1];
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const float x0 = __uint_as_float(w[e] << 16) * sc, x1 = __uint_as_float(w[e] & 0xFFFF0000u) * sc;
-                        hi[e] = split2(x0, x1, lo[e]);
-                    }
-                    const uint32_t off = half * SBO_V + (j >> 3) * 128 + (j & 7) * 16;
-                    *reinterpret_cast<uint4*>(vt + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-                    *reinterpret_cast<uint4*>(vt + 2 * SBO_V + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+            for (int it = 0; it < 2 * C / kVtThreads; ++it) {
+                const int idx = tid_v + it * kVtThreads, j = idx >> 1, half = idx & 1;
+                const uint32_t voff = j * 32 + ((half ^ ((j >> 2) & 1)) * 16);   // undo 32B swizzle
+                const uint4 raw = *reinterpret_cast<const uint4*>(vs + voff);
+                *reinterpret_cast<uint4*>(vt + L::vc_off + voff) = raw;          // the V tile itself, same (swizzled) placement: O2's operand
+                const float sc = ex2(b_last - b2[j]);
+                const uint32_t w[4] = {raw.x, raw.y, raw.z, raw.w};
+                uint32_t hi[4], lo[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const float x0 = __uint_as_float(w[e] << 16) * sc, x1 = __uint_as_float(w[e] & 0xFFFF0000u) * sc;
+                    hi[e] = split2(x0, x1, lo[e]);
                 }
+                const uint32_t off = half * SBO_V + (j >> 3) * 128 + (j & 7) * 16;
+                *reinterpret_cast<uint4*>(vt + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+                *reinterpret_cast<uint4*>(vt + 2 * SBO_V + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
             }
-            mbar_wait(&bars[BI.p_full + pb], (c / NB) & 1);
-            tc_fence_after_sync();
-            uint8_t* ah = sm + L::a_off + pb * 2 * L::a_bytes;
-            // 16-row group of this warp: row r of an M=64 tile sits in TMEM lane 32(r/16) + r%16, of an M=128 tile in lane r
-            const int rg = kAlt ? q : 2 * q + (int)wg;
-            const uint32_t lane_base = kAlt ? 32 * q : 32 * q + 16 * wg;
-            const int ra = 16 * rg + (lane >> 2), rb = ra + 8;
-            const float ba = b2[ra], bb = b2[rb];
-            // UMMA A operand, K-major interleaved: (i,j) -> (i/8)*SBO_A + (j/8)*128 + (i%8)*16 + (j%8)*2
-            uint8_t* arow = ah + (ra >> 3) * SBO_A + (ra & 7) * 16 + (lane & 3) * 4;
-#pragma unroll
-            for (int cp = 0; cp < C / 32; ++cp) {   // two 16-column blocks per pass
-                if (2 * cp <= rg) {
-                    uint32_t r[2][8];
-                    tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_p + pb * C + (2 * cp) * 16), r[0]);
-                    if (2 * cp + 1 <= rg) tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_p + pb * C + (2 * cp + 1) * 16), r[1]);
-                    tmem_ld_wait();
-                    if (2 * cp + 2 > rg) {   // last pass of this warp: P(c) is in registers, the TMEM buffer may be overwritten
-                        tc_fence_before_sync();
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(&bars[BI.p_empty + pb]);
-                    }
-#pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const int cb = 2 * cp + u;
-                        if (cb <= rg) {
-#pragma unroll
-                            for (int jb = 0; jb < 2; ++jb) {
-                                const int j0 = cb * 16 + jb * 8 + 2 * (lane & 3);
-                                const float2 bj = *reinterpret_cast<const float2*>(b2 + j0);
-                                float a0 = __uint_as_float(r[u][4 * jb + 0]) * ex2(ba - bj.x);
-                                float a1 = __uint_as_float(r[u][4 * jb + 1]) * ex2(ba - bj.y);
-                                float c0 = __uint_as_float(r[u][4 * jb + 2]) * ex2(bb - bj.x);
-                                float c1 = __uint_as_float(r[u][4 * jb + 3]) * ex2(bb - bj.y);
-                                if (cb == rg) {   // diagonal block: causal mask j <= i
-                                    a0 = (j0 <= ra) ? a0 : 0.f;
-                                    a1 = (j0 + 1 <= ra) ? a1 : 0.f;
-                                    c0 = (j0 <= rb) ? c0 : 0.f;
-                                    c1 = (j0 + 1 <= rb) ? c1 : 0.f;
-                                }
-                                uint32_t lo_a, lo_c;
-                                const uint32_t hi_a = split2(a0, a1, lo_a), hi_c = split2(c0, c1, lo_c);
-                                uint8_t* pa = arow + (cb * 2 + jb) * 128;
-                                *reinterpret_cast<uint32_t*>(pa) = hi_a;
-                                *reinterpret_cast<uint32_t*>(pa + L::a_bytes) = lo_a;
-                                *reinterpret_cast<uint32_t*>(pa + SBO_A) = hi_c;              // row + 8
-                                *reinterpret_cast<uint32_t*>(pa + SBO_A + L::a_bytes) = lo_c;
-                            }
-                        }
-                    }
-                }
-            }
-            fence_proxy_async_smem();   // generic-proxy writes of A, V~ -> visible to tcgen05.mma's operand reads
+            fence_proxy_async_smem();   // generic-proxy writes -> visible to tcgen05.mma's operand reads
             __syncwarp();
-            if (q == 3 && lane == 0) TC_TRACE(6, c);
             if (lane == 0) {
-                mbar_arrive(&bars[BI.a_full + pb]);
-                mbar_arrive(&bars[BI.empty + s]);
-                const bool last_in_batch = kAlt ? ((c % CPB) + 2 >= (uint32_t)CPB || c + 2 >= n_chunks)
-                                                : ((c % CPB) == (uint32_t)CPB - 1 || c + 1 == n_chunks);
-                if (last_in_batch) mbar_arrive(&bars[BI.g_empty + gslot]);
+                mbar_arrive(&bars[BI.vt_full + pb]);
+                if ((c % CPB) == (uint32_t)CPB - 1 || c + 1 == n_chunks) mbar_arrive(&bars[BI.g_empty + gslot]);
             }
         }
+    }
+    else if (warp >= 8 && warp < 12) {
+        // ================= score warps: A[:, slice] = P[:, slice] ⊙ 2^(b_i - b_j) (causal) -> every CTA of the cluster =================
+        // One warp per TMEM lane quadrant.  A quadrant holds 16 rows of an M = 64 tile (row r in lane 32(r/16) + r%16) or 32
+        // rows of an M = 128 tile (row r in lane r): NG 16-row groups per warp.  A group whose rows all precede the slice's
+        // first key is entirely above the diagonal: it is skipped here and never written anywhere (it stays zero).
+        constexpr int NG = C / 64;
+        constexpr uint32_t kSlice = (NA / 8) * L::a_lbo;           // bytes of one CTA's slice
+        constexpr uint32_t tx = (CS - 1) * kSlice;                  // what the peers push into this CTA's A buffer per chunk
+        auto rows_base = [&](int qq, int gi) { return (C == 64) ? 16 * qq : 32 * qq + 16 * gi; };
+        bool act[NG];
+#pragma unroll
+        for (int gi = 0; gi < NG; ++gi) act[gi] = (uint32_t)rows_base(q, gi) + 15 >= key0;
+        for (uint32_t c = 0; c < n_chunks; ++c) {
+            const uint32_t pb = c % NB, bt = c / CPB, gslot = bt & 1;
+            mbar_wait(&bars[BI.g_full + gslot], (bt >> 1) & 1);
+            const float* b2 = gate + gslot * 2 * kGateBatch + (c % CPB) * C;
+            if (q == 3 && lane == 0) TC_TRACE(5, c);
+            // every b_j is read before the first A store (the stores may alias b2 as far as the compiler can tell)
+            float2 bj[NA / 8];
+#pragma unroll
+            for (int jb = 0; jb < NA / 8; ++jb) bj[jb] = *reinterpret_cast<const float2*>(b2 + key0 + jb * 8 + 2 * (lane & 3));
+            float bi[NG][2];
+#pragma unroll
+            for (int gi = 0; gi < NG; ++gi) {
+                bi[gi][0] = b2[rows_base(q, gi) + (lane >> 2)];
+                bi[gi][1] = b2[rows_base(q, gi) + (lane >> 2) + 8];
+            }
+            mbar_wait(&bars[BI.a_empty + pb], ((c / NB) & 1) ^ 1);   // all CS CTAs are done reading A buffer pb (chunk c - NB)
+            mbar_wait(&bars[BI.p_full + pb], (c / NB) & 1);
+            tc_fence_after_sync();
+            uint32_t r[NG][NA / 2];
+#pragma unroll
+            for (int gi = 0; gi < NG; ++gi)
+                if (act[gi]) tmem_ld_slice<NA>(tmem_addr(tb, (C == 64) ? 32 * q : 32 * q + 16 * gi, L::tm_p + pb * 32), r[gi]);
+            tmem_ld_wait();
+            tc_fence_before_sync();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars[BI.p_empty + pb]);   // this warp's part of P(c) is in registers
+            uint8_t* ab = sm + L::a_off + pb * L::a_bytes;
+#pragma unroll
+            for (int gi = 0; gi < NG; ++gi) {
+                if (act[gi]) {
+                    const int ra = rows_base(q, gi) + (lane >> 2), rb = ra + 8;
+                    uint32_t hi_a[NA / 8], lo_a[NA / 8], hi_c[NA / 8], lo_c[NA / 8];
+#pragma unroll
+                    for (int jb = 0; jb < NA / 8; ++jb) {
+                        const int j0 = (int)key0 + jb * 8 + 2 * (lane & 3);
+                        float a0 = __uint_as_float(r[gi][4 * jb + 0]) * ex2(bi[gi][0] - bj[jb].x);
+                        float a1 = __uint_as_float(r[gi][4 * jb + 1]) * ex2(bi[gi][0] - bj[jb].y);
+                        float c0 = __uint_as_float(r[gi][4 * jb + 2]) * ex2(bi[gi][1] - bj[jb].x);
+                        float c1 = __uint_as_float(r[gi][4 * jb + 3]) * ex2(bi[gi][1] - bj[jb].y);
+                        a0 = (j0 <= ra) ? a0 : 0.f;       // causal mask j <= i
+                        a1 = (j0 + 1 <= ra) ? a1 : 0.f;
+                        c0 = (j0 <= rb) ? c0 : 0.f;
+                        c1 = (j0 + 1 <= rb) ? c1 : 0.f;
+                        hi_a[jb] = split2(a0, a1, lo_a[jb]);
+                        hi_c[jb] = split2(c0, c1, lo_c[jb]);
+                    }
+                    uint8_t* arow = ab + (ra >> 3) * 128 + (ra & 7) * 16 + (lane & 3) * 4;
+#pragma unroll
+                    for (int jb = 0; jb < NA / 8; ++jb) {
+                        uint8_t* pa = arow + (key0 / 8 + jb) * L::a_lbo;
+                        *reinterpret_cast<uint32_t*>(pa) = hi_a[jb];
+                        *reinterpret_cast<uint32_t*>(pa + L::a_term) = lo_a[jb];
+                        *reinterpret_cast<uint32_t*>(pa + 128) = hi_c[jb];              // row + 8
+                        *reinterpret_cast<uint32_t*>(pa + 128 + L::a_term) = lo_c[jb];
+                    }
+                }
+            }
+            fence_proxy_async_smem();   // generic-proxy writes of A -> visible to the bulk copies and to tcgen05.mma
+            __syncwarp();
+            // the slice of this CTA (all rows, both terms: NA/8 consecutive 8-key groups) is one contiguous range of the A
+            // buffer: once the four score warps have written it, one lane per peer pushes it into the same place of that
+            // peer's buffer pb; the copy completes (tx bytes) on the peer's a_full barrier
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            if (q == 0 && lane < CS - 1) {
+                const uint32_t d = (uint32_t)lane + ((uint32_t)lane >= rank ? 1u : 0u);
+                const uint32_t off = L::a_off + pb * L::a_bytes + (key0 / 8) * L::a_lbo;
+                bulk_copy_to_cluster(mapa(sm_a + off, d), sm_a + off, kSlice, mapa(smem_u32(&bars[BI.a_full + pb]), d));
+            }
+            if (q == 3 && lane == 0) TC_TRACE(6, c);
+            if (lane == 0) {
+                if (q == 3) mbar_arrive_expect_tx(&bars[BI.a_full + pb], tx);   // quadrant 3 holds the last rows: always active
+                else mbar_arrive(&bars[BI.a_full + pb]);
+                if ((c % CPB) == (uint32_t)CPB - 1 || c + 1 == n_chunks) mbar_arrive(&bars[BI.g_empty + gslot]);
+            }
+        }
+        // tail: the peers' last O2 commits have reached this CTA's barriers before anyone may exit
+        for (uint32_t c = n_chunks > (uint32_t)NB ? n_chunks - NB : 0; c < n_chunks; ++c)
+            mbar_wait(&bars[BI.a_empty + c % NB], (c / NB) & 1);
     } else if (st_warp) {
         // ================= state warps: the carry  S <- 2^(b_C) S + (Uh + Ul), fp32 FMA in registers =================
+#pragma unroll
+        for (int j = 0; j < 16; ++j) S[j] = 0.f;
+        if (st_active && state_in) {
+            const float4* p = reinterpret_cast<const float4*>(state_in + ((size_t)bh * DK + krow) * DV + dv0);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float4 x = p[j];
+                S[4 * j] = x.x; S[4 * j + 1] = x.y; S[4 * j + 2] = x.z; S[4 * j + 3] = x.w;
+            }
+        }
+        write_s_operand(0);   // version 0 of the S operand (read by O1(0))
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars[BI.s_full]);
         for (uint32_t c = 0; c < n_chunks; ++c) {
             const uint32_t ob = c & 1, bt = c / CPB, gslot = bt & 1;
             mbar_wait(&bars[BI.g_full + gslot], (bt >> 1) & 1);
@@ -530,8 +617,8 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             const uint32_t ob = c & 1, bt = c / CPB, gslot = bt & 1;
             mbar_wait(&bars[BI.g_full + gslot], (bt >> 1) & 1);
             const float* eb = gate + gslot * 2 * kGateBatch + kGateBatch + (c % CPB) * C;
-            mbar_wait(&bars[BI.o2_full + ob], (c >> 1) & 1);
-            mbar_wait(&bars[BI.o1_full + ob], (c >> 1) & 1);
+            mbar_wait_relaxed(&bars[BI.o2_full + ob], (c >> 1) & 1);
+            mbar_wait_relaxed(&bars[BI.o1_full + ob], (c >> 1) & 1);
             tc_fence_after_sync();
             const uint64_t t0 = (uint64_t)c * C;
             const int n = (int)((T - t0) < (uint64_t)C ? (T - t0) : (uint64_t)C);
@@ -569,9 +656,12 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
         }
     }
 
-    // ---- teardown: every tcgen05 op has completed (the state and epilogue warps waited on the last commits) ----
+    // ---- teardown: every tcgen05 op of this CTA has completed (the state and epilogue warps waited on the last commits),
+    // and no peer still multicasts, copies or arrives into this CTA once the whole cluster is here ----
     tc_fence_before_sync();
-    __syncthreads();
+    if (threadIdx.x == 0) TC_TRACE(11, 0);
+    cluster_sync();
+    if (threadIdx.x == 0) TC_TRACE(12, 0);
     if (warp == 2) tmem_dealloc(tb, L::tmem_cols);
 }
 
@@ -593,7 +683,7 @@ static TmapEncodeFn tmap_encode_fn() {
 }
 
 // 4-D map over a [B, t_stride, H, D] bf16 tensor whose first `T` tokens per batch row are valid:
-// dims (D, H, T, B), box (box_d, 1, C, 1).  Rows beyond T read as zero (the short last chunk).
+// dims (D, H, T, B), box (box_d, 1, box_t, 1).  Rows beyond T read as zero (the short last chunk).
 static int make_tmap(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, uint64_t T, uint64_t t_stride, uint32_t B,
                      uint32_t box_d, uint32_t box_t, CUtensorMapSwizzle sw) {
     TmapEncodeFn enc = tmap_encode_fn();
@@ -608,13 +698,13 @@ static int make_tmap(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, u
     return r == CUDA_SUCCESS ? ESC_OK : ESC_ERR_CUDA;
 }
 
-template <int DK, int C, typename OutT>
+template <int DK, int C, int CS, typename OutT>
 static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                        float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
     using L = TcCfg<DK, C>;
     static bool attr_set = false;
     if (!attr_set) {
-        ESC_CUDA(cudaFuncSetAttribute(esc_scan_tc_kernel<DK, C, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::total));
+        ESC_CUDA(cudaFuncSetAttribute(esc_scan_tc_kernel<DK, C, CS, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::total));
         attr_set = true;
     }
     if (!state_out) return ESC_OK;   // prepare-only call (before a stream capture)
@@ -622,36 +712,80 @@ static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const v
     const void* qq = T ? q : (const void*)state_out;   // T == 0: maps are never dereferenced, any valid address will do
     const void* kk = T ? k : (const void*)state_out;
     const void* vv = T ? v : (const void*)state_out;
-    int rc = make_tmap(&tq, qq, DK, s.H, T, t_stride ? t_stride : 1, s.B, 64, C, CU_TENSOR_MAP_SWIZZLE_128B);
-    if (rc == ESC_OK) rc = make_tmap(&tk, kk, DK, s.H, T, t_stride ? t_stride : 1, s.B, 64, C, CU_TENSOR_MAP_SWIZZLE_128B);
+    // Q / K: each CTA of the cluster loads (and multicasts) C / CS rows of a chunk; V: the CTA's own 16 columns
+    int rc = make_tmap(&tq, qq, DK, s.H, T, t_stride ? t_stride : 1, s.B, 64, C / CS, CU_TENSOR_MAP_SWIZZLE_128B);
+    if (rc == ESC_OK) rc = make_tmap(&tk, kk, DK, s.H, T, t_stride ? t_stride : 1, s.B, 64, C / CS, CU_TENSOR_MAP_SWIZZLE_128B);
     if (rc == ESC_OK) rc = make_tmap(&tv, vv, s.dv, s.H, T, t_stride ? t_stride : 1, s.B, kTcDVT, C, CU_TENSOR_MAP_SWIZZLE_32B);
     if (rc != ESC_OK) return rc;
-    dim3 grid(s.dv / kTcDVT, s.B * s.H);
-    esc_scan_tc_kernel<DK, C, OutT><<<grid, kTcThreads, L::total, stream>>>(tq, tk, tv, g, state_in, state_out, (OutT*)o, s.H,
-                                                                             s.dv, T, t_stride);
-    ESC_CUDA(cudaGetLastError());
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(s.dv / kTcDVT, s.B * s.H);   // d_v / 16 CTAs per (b, h), in clusters of CS
+    cfg.blockDim = dim3(kTcThreads);
+    cfg.dynamicSmemBytes = L::total;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[2];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CS;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.* in the kernel
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 2;
+    ESC_CUDA(cudaLaunchKernelEx(&cfg, esc_scan_tc_kernel<DK, C, CS, OutT>, tq, tk, tv, g, state_in, state_out, (OutT*)o, s.H, s.dv, T,
+                                t_stride));
     return ESC_OK;
 }
 
-template <int DK, int C>
+template <int DK, int C, int CS>
 static int launch_tc_o(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                        float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
-    if (s.out_dtype == ESC_DTYPE_F32) return launch_tc_t<DK, C, float>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
-    return launch_tc_t<DK, C, bf16>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.out_dtype == ESC_DTYPE_F32) return launch_tc_t<DK, C, CS, float>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    return launch_tc_t<DK, C, CS, bf16>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+}
+
+// Cluster size: 4.  A cluster of 8 (all d_v slices of a d_v = 128 head) would share twice as much, but B200 can keep only 15
+// such clusters resident at this shared-memory footprint (cudaOccupancyMaxActiveClusters, r01): the 16 heads of the B = 1
+// workloads would run as two waves.  Clusters of 4 fit 33 times: 32 clusters (128 CTAs) in one wave.
+constexpr int kTcCluster = 4;
+
+template <int DK, int C>
+static int launch_tc_dv(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
+                        float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
+    if (s.dv % (kTcDVT * kTcCluster)) return ESC_ERR_UNSUPPORTED;
+    return launch_tc_o<DK, C, kTcCluster>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
 }
 
 int launch_scan_tc(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                    float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
-    if (s.dk == 128 && s.chunk == 64) return launch_tc_o<128, 64>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
-    if (s.dk == 128 && s.chunk == 128) return launch_tc_o<128, 128>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
-    if (s.dk == 64 && s.chunk == 64) return launch_tc_o<64, 64>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
-    if (s.dk == 64 && s.chunk == 128) return launch_tc_o<64, 128>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 128 && s.chunk == 64) return launch_tc_dv<128, 64>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 128 && s.chunk == 128) return launch_tc_dv<128, 128>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 64 && s.chunk == 64) return launch_tc_dv<64, 64>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 64 && s.chunk == 128) return launch_tc_dv<64, 128>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
     return ESC_ERR_UNSUPPORTED;
 }
 
 #ifdef ESC_TC_TRACE
 extern "C" int esc_debug_trace_read(long long* host) {
     return (int)cudaMemcpyFromSymbol(host, g_tc_trace, sizeof(g_tc_trace));
+}
+extern "C" int esc_debug_max_clusters(int* out8, int* out4) {
+    using L = TcCfg<128, 64>;
+    cudaLaunchConfig_t cfg = {};
+    cfg.blockDim = dim3(kTcThreads);
+    cfg.dynamicSmemBytes = L::total;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaFuncSetAttribute(esc_scan_tc_kernel<128, 64, 4, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::total);
+    cudaFuncSetAttribute(esc_scan_tc_kernel<128, 64, 4, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::total);
+    attr[0].val.clusterDim.x = 4; cfg.gridDim = dim3(8, 64);
+    cudaError_t e = cudaOccupancyMaxActiveClusters(out8, esc_scan_tc_kernel<128, 64, 4, float>, &cfg);
+    attr[0].val.clusterDim.x = 4; cfg.gridDim = dim3(4, 64);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(out4, esc_scan_tc_kernel<128, 64, 4, float>, &cfg);
+    return (int)e;
 }
 #endif
 
