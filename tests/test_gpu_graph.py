@@ -120,3 +120,64 @@ def test_cold_plan_graph_matches_direct_calls(esc, ctx):
     for (eo, es_), o, s in zip(exp, outs, st):
         assert bits_equal(o, eo) and bits_equal(s, es_)
     graph.destroy()
+
+
+def test_config3_fork_continue_rollback_replay(esc, ctx):
+    # BASELINE config 3: one 8k-prefix capsule of the 24-layer hybrid layout forked into 8 sessions in device memory, each
+    # continued with 128 distinct seeded suffix tokens, then rolled back to the capsule and replayed: states, outputs and
+    # the capsule's valid ranges byte-identical to the first pass.
+    from paper_2606_20537_b200 import workload
+    P, n_sess, suffix = 8192, 8, 128
+    key = esc.shape_key_make(B, H, DK, DV, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
+    src = workload.HybridSession(ctx, P + suffix, seed=40, device=DEV)
+    slab = src.new_slab(P)
+    src.set.set_position(P)
+    cap = esc.snapshot(src.set, P, CHUNK, slab)
+    assert cap.info().payload_bytes == 18 * (1 << 20) + 24576 * P      # 210 MiB
+    sessions = [workload.HybridSession(ctx, P + suffix, seed=41 + i, device=DEV) for i in range(n_sess)]
+    inputs = [workload.SuffixInputs(len(src.lin), suffix, seed=60 + i, device=DEV) for i in range(n_sess)]
+    esc.fork(cap, [s.set for s in sessions])
+    torch.cuda.synchronize()
+    for s in sessions:            # every session's valid ranges == the source's, byte for byte
+        for spec, a, b_ in zip(s.specs, s.bufs, src.bufs):
+            nv = spec.fixed_bytes + P * spec.bytes_per_token
+            assert torch.equal(a.view(torch.uint8).view(-1)[:nv], b_.view(torch.uint8).view(-1)[:nv]), spec.name
+
+    def continue_all():
+        res = []
+        for s, inp in zip(sessions, inputs):
+            for n in range(len(s.lin)):
+                q, k, v, g = inp.dev[n]
+                esc.linattn_scan(ctx, key, q, k, v, g, s.states[n], s.states[n], inp.out[n], suffix, suffix, CHUNK)
+            # the harness "appends" 128 KV tokens: dirties [P, P+128) of every KV row
+            for spec, buf in zip(s.specs, s.bufs):
+                if spec.bytes_per_token:
+                    buf.view(torch.uint8).view(-1)[P * spec.bytes_per_token:(P + suffix) * spec.bytes_per_token].fill_(0x5A)
+            s.set.set_position(P + suffix)
+        torch.cuda.synchronize()
+        for s, inp in zip(sessions, inputs):
+            res.append(([st.clone() for st in s.states], inp.out_dev.clone()))
+        return res
+
+    first = continue_all()
+    assert not bits_equal(first[0][0][0], first[1][0][0])            # distinct suffixes: the branches differ
+    for s in sessions:
+        esc.rollback(s.set, cap)
+        assert s.set.position == P
+    torch.cuda.synchronize()
+    for s in sessions:
+        for n, st in enumerate(s.states):
+            assert bits_equal(st, src.states[n])
+    for inp in inputs:
+        inp.out_dev.fill_(0xFF)
+    second = continue_all()
+    for (st1, o1), (st2, o2) in zip(first, second):
+        assert torch.equal(o1, o2)
+        for a, b_ in zip(st1, st2):
+            assert bits_equal(a, b_)
+    # one branch against the oracle (state_in = the capsule's fold state)
+    si = synth.scan_inputs(B, suffix, H, DK, DV, seed_ids=(31, 60 + 3, 5))
+    qf, kf, vf, gf = si.as_f32()
+    o_ref, s_ref = oracle.linattn_recurrence(qf, kf, vf, gf, src.states[5].cpu().numpy().astype(np.float64))
+    assert err_o(inputs[3].out[5].cpu().numpy(), o_ref) <= TOL_O
+    assert err_s(second[3][0][5].cpu().numpy(), s_ref) <= TOL_S

@@ -186,3 +186,61 @@ def test_full_size_config2_sampled(esc, ctx):
     o_ref, s_ref = oracle.linattn_recurrence(q[:, :, heads], k[:, :, heads], v[:, :, heads], g[:, :, heads])
     assert err_o(o[:, :, heads].cpu().numpy(), o_ref) <= TOL_O
     assert err_s(s[:, heads].cpu().numpy(), s_ref) <= TOL_S
+
+
+@pytest.mark.parametrize("B,T,chunk", [
+    (4, 2048, 64),      # 64 (b,h) scans = 128 clusters: several waves of CTAs on 148 SMs
+    (2, 8192, 128),
+    (1, 32768, 64),
+])
+def test_config4_sweep_points_sampled(esc, ctx, B, T, chunk):
+    # BASELINE config 4 (scan sweep: B 1-4, H16, d128, T 2k-64k, chunk 64/128) at full head shape: the oracle checks a
+    # seeded sample of (b, h) scans over the whole sequence; a chunk-aligned boundary at T/2 must continue bit-identically
+    # to the cold run, a misaligned one (T/2 + 37) within tolerance.
+    H, dk, dv = 16, 128, 128
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(17, B, T, chunk))
+    dev_in = scan_dev_inputs(si)
+    o_cold, s_cold, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk)
+    q, k, v, g = si.as_f32()
+    for (b, h) in [(0, 0), (B - 1, 9), (B // 2, 15)]:
+        sl = (slice(b, b + 1), slice(None), slice(h, h + 1))
+        o_ref, s_ref = oracle.linattn_recurrence(q[sl], k[sl], v[sl], g[sl])
+        assert err_o(o_cold[b:b + 1, :, h:h + 1].cpu().numpy(), o_ref) <= TOL_O
+        assert err_s(s_cold[b:b + 1, h:h + 1].cpu().numpy(), s_ref) <= TOL_S
+        # misaligned restore of this (b, h): oracle tolerance only
+    P = (T // 2) // chunk * chunk
+    _, s_p, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, n=P)
+    o_b, s_t, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=s_p, t0=P)
+    assert bits_equal(o_b, o_cold[:, P:]) and bits_equal(s_t, s_cold)
+    Pm = P + 37
+    _, s_pm, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, n=Pm)
+    o_m, s_tm, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=s_pm, t0=Pm)
+    b, h = B - 1, 9
+    sl = (slice(b, b + 1), slice(None), slice(h, h + 1))
+    o_ref, s_ref = oracle.linattn_recurrence(q[sl], k[sl], v[sl], g[sl])
+    assert err_o(o_m[b:b + 1, :, h:h + 1].cpu().numpy(), o_ref[:, Pm:]) <= TOL_O
+    assert err_s(s_tm[b:b + 1, h:h + 1].cpu().numpy(), s_ref) <= TOL_S
+
+
+def test_back_to_back_scans_on_one_stream_are_ordered(esc, ctx):
+    # the scan kernel allows programmatic dependent launch: a following scan may start its on-chip setup early but must
+    # not read the state the previous one is still writing.  20 chained in-place suffix scans == one scan over all tokens.
+    B, H, dk, dv, chunk, n, T = 1, 16, 128, 128, 64, 20, 20 * 64
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(18,), gate="slow")
+    dev_in = scan_dev_inputs(si)
+    o_cold, s_cold, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk)
+    key = esc.shape_key_make(B, H, dk, dv, esc.DTYPE_BF16, esc.DTYPE_F32, chunk)
+    q, k, v, g = dev_in
+    state = torch.zeros((B, H, dk, dv), dtype=torch.float32, device=DEV)
+    o = torch.zeros((B, T, H, dv), dtype=torch.float32, device=DEV)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    for rep in range(3):
+        state.zero_()
+        stream.wait_stream(torch.cuda.current_stream())
+        for i in range(n):
+            t0 = i * 64
+            esc.linattn_scan(ctx, key, q[:, t0:], k[:, t0:], v[:, t0:], g[:, t0:], state, state, o[:, t0:], 64, T, chunk,
+                             stream=stream)
+        stream.synchronize()
+        assert bits_equal(o, o_cold) and bits_equal(state, s_cold)
