@@ -419,6 +419,35 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
         cap.destroy()
         del full, slab
         torch.cuda.empty_cache()
+    # ---- host tier: demote / promote / restore straight from the pinned host slab, 66 MiB capsule ----
+    sess2 = workload.HybridSession(ctx, P_STEP + SUFFIX, seed=9, device=dev)
+    slab = sess2.new_slab(P_STEP)
+    sess2.set.set_position(P_STEP)
+    cap = esc.snapshot(sess2.set, P_STEP, CHUNK, slab, stream=stream)
+    pay = cap.info().payload_bytes
+    host = torch.empty(slab.numel(), dtype=torch.uint8).pin_memory()
+    slab2 = sess2.new_slab(P_STEP)
+    hcaps, gcaps = [], []
+
+    def demote():
+        hcaps.append(esc.capsule_demote(cap, host, stream=stream))
+    demote_ms, _ = med_ms(demote, n=7)
+
+    def promote():
+        gcaps.append(esc.capsule_promote(hcaps[0], slab2, stream=stream))
+    promote_ms, _ = med_ms(promote, n=7)
+    host_restore_ms, _ = med_ms(lambda: esc.restore(sess2.set, hcaps[0], stream=stream), n=7)
+    with torch.cuda.stream(stream):
+        link_ms, _ = med_ms(lambda: slab2.copy_(host, non_blocking=True), n=7)
+    res["host_tier"] = {"capsule_MiB": pay / 2**20,
+                        "demote_ms": demote_ms, "demote_GBps": pay / (demote_ms * 1e-3) / 1e9,
+                        "promote_ms": promote_ms, "promote_GBps": pay / (promote_ms * 1e-3) / 1e9,
+                        "restore_from_host_ms": host_restore_ms, "restore_from_host_GBps": pay / (host_restore_ms * 1e-3) / 1e9,
+                        "link_h2d_GBps_torch_copy": slab2.numel() / (link_ms * 1e-3) / 1e9,
+                        "note": "GB/s = capsule payload bytes crossing the host link once / time; restore_from_host = the copy kernel "
+                                "reading the pinned slab in place (promotion fused into restore); link = torch pinned H2D copy of the slab"}
+    for c in hcaps + gcaps + [cap]:
+        c.destroy()
     res["warm_vs_cold"] = {"note": "cold = 18 layers x scan(T=P+64) in one graph; warm = one graph [restore(P) + 18 x scan(64)]; "
                                    "median of 15 (7 at 16k), L2 flushed; the scan only — the paper's TTFT includes the whole model",
                            "by_prefix": table}

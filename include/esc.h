@@ -179,12 +179,32 @@ typedef struct esc_capsule_info {
     uint32_t n_rows;
     uint32_t n_segments;      /* rows x segments = entries of the copy table      */
     uint32_t aligned;         /* 1 when boundary % chunk == 0 (or chunk == 0)     */
-    uint32_t reserved;
+    uint32_t tier;            /* ESC_TIER_GPU or ESC_TIER_HOST                     */
 } esc_capsule_info;
 int esc_capsule_info_get(const esc_bufset* capsule, esc_capsule_info* out_info);
 /* Valid end (bytes per segment) of row `row` at the capsule's boundary (PAPER.md:86
  * "valid ends" in the descriptor). */
 int esc_capsule_valid_end(const esc_bufset* capsule, uint32_t row, uint64_t* out_bytes_per_segment);
+
+/* ---- tiers (Algorithm 1: "return tiered handle" PAPER.md:122, "promote if off-GPU" PAPER.md:125-126) ----
+ * The one mechanism the capsule adds to the contract is "host-backed buffers and cross-space asynchronous
+ * copy"; which capsule lives where, and when, is serving policy and stays
+ * with the caller.  A capsule's storage slab is ONE contiguous range, so a tier move is one async copy.
+ *   demote : GPU-tier capsule -> caller-owned PINNED host storage (cudaHostAlloc / cudaHostRegister / torch
+ *            pin_memory; ESC_ERR_INVALID for pageable memory), one async D2H copy of slab_bytes on `stream`.
+ *            Returns a HOST-tier capsule handle; the GPU-tier one stays valid (the caller frees its slab
+ *            when it wants the memory back).
+ *   promote: HOST-tier capsule -> caller-owned device storage (256-B aligned), one async H2D copy.
+ * esc_restore / esc_rollback / esc_fork / esc_graph_set_capsule also take a HOST-tier capsule directly: the
+ * copy kernel then reads the pinned slab over the host link (zero-copy), i.e. promotion is fused into the
+ * restore and the bytes cross the link once and land in place — "promotion is the only non-sub-ms step"
+ * (PAPER.md:161).  Same layout, digests, boundary and byte-exactness as the GPU tier. */
+#define ESC_TIER_GPU  0u
+#define ESC_TIER_HOST 1u
+int esc_capsule_demote(const esc_bufset* capsule, void* storage_host, uint64_t storage_bytes, void* stream,
+                       esc_bufset** out_host_capsule);
+int esc_capsule_promote(const esc_bufset* host_capsule, void* storage_dev, uint64_t storage_bytes, void* stream,
+                        esc_bufset** out_capsule);
 
 /* ---- chunked gated linear-attention scan ---------------------------------------------- */
 #define ESC_DTYPE_BF16 1u

@@ -152,6 +152,8 @@ int esc_bufset_create(esc_ctx* ctx, const esc_buf_desc* descs, uint32_t n_rows, 
     s->layout_digest = layout_digest(s->rows);
     s->position = ESC_POSITION_UNKNOWN;
     s->slab = nullptr;
+    s->slab_host = nullptr;
+    s->tier = ESC_TIER_GPU;
     s->slab_bytes = s->payload_bytes = s->chunk = s->prefix_digest = 0;
     *out_set = s;
     return ESC_OK;
@@ -221,6 +223,8 @@ int esc_snapshot(esc_bufset* live, uint64_t P, uint64_t chunk, uint64_t prefix_d
     cap->layout_digest = live->layout_digest;
     cap->position = P;
     cap->slab = (uint8_t*)storage_dev;
+    cap->slab_host = nullptr;
+    cap->tier = ESC_TIER_GPU;
     cap->slab_bytes = slab_bytes;
     cap->payload_bytes = payload;
     cap->chunk = chunk;
@@ -314,6 +318,64 @@ int esc_capsule_info_get(const esc_bufset* capsule, esc_capsule_info* out_info) 
     for (const Row& r : capsule->rows) ns += r.n_seg;
     out_info->n_segments = ns;
     out_info->aligned = (capsule->chunk == 0 || capsule->position % capsule->chunk == 0) ? 1u : 0u;
+    out_info->tier = capsule->tier;
+    return ESC_OK;
+}
+
+// ---- tiers: a capsule slab is one contiguous range, a tier move is one async copy ----
+static esc_bufset* clone_capsule(const esc_bufset* c) {
+    esc_bufset* n = new (std::nothrow) esc_bufset(*c);
+    return n;
+}
+
+int esc_capsule_demote(const esc_bufset* capsule, void* storage_host, uint64_t storage_bytes, void* stream,
+                       esc_bufset** out_host_capsule) {
+    if (!capsule || !capsule->frozen || capsule->tier != ESC_TIER_GPU || !storage_host || !out_host_capsule)
+        return ESC_ERR_INVALID;
+    if (storage_bytes < capsule->slab_bytes) return ESC_ERR_CAPACITY;
+    if (((uintptr_t)storage_host & 255u) != 0) return ESC_ERR_UNALIGNED;
+    // the storage must be pinned and mapped: the restore kernels read it in place
+    cudaPointerAttributes at;
+    ESC_CUDA(cudaPointerGetAttributes(&at, storage_host));
+    if (at.type != cudaMemoryTypeHost || !at.devicePointer) return ESC_ERR_INVALID;
+    esc_bufset* h = clone_capsule(capsule);
+    if (!h) return ESC_ERR_INVALID;
+    h->tier = ESC_TIER_HOST;
+    h->slab_host = (uint8_t*)storage_host;
+    h->slab = (uint8_t*)at.devicePointer;
+    cudaError_t e = capsule->slab_bytes
+                        ? cudaMemcpyAsync(storage_host, capsule->slab, capsule->slab_bytes, cudaMemcpyDeviceToHost, (cudaStream_t)stream)
+                        : cudaSuccess;
+    if (e != cudaSuccess) {
+        delete h;
+        return cuda_fail(e);
+    }
+    *out_host_capsule = h;
+    return ESC_OK;
+}
+
+int esc_capsule_promote(const esc_bufset* host_capsule, void* storage_dev, uint64_t storage_bytes, void* stream,
+                        esc_bufset** out_capsule) {
+    if (!host_capsule || !host_capsule->frozen || host_capsule->tier != ESC_TIER_HOST || !storage_dev || !out_capsule)
+        return ESC_ERR_INVALID;
+    if (storage_bytes < host_capsule->slab_bytes) return ESC_ERR_CAPACITY;
+    if (((uintptr_t)storage_dev & 255u) != 0) return ESC_ERR_UNALIGNED;
+    cudaPointerAttributes at;
+    ESC_CUDA(cudaPointerGetAttributes(&at, storage_dev));
+    if (at.type != cudaMemoryTypeDevice) return ESC_ERR_INVALID;
+    esc_bufset* g = clone_capsule(host_capsule);
+    if (!g) return ESC_ERR_INVALID;
+    g->tier = ESC_TIER_GPU;
+    g->slab_host = nullptr;
+    g->slab = (uint8_t*)storage_dev;
+    cudaError_t e = host_capsule->slab_bytes ? cudaMemcpyAsync(storage_dev, host_capsule->slab_host, host_capsule->slab_bytes,
+                                                               cudaMemcpyHostToDevice, (cudaStream_t)stream)
+                                             : cudaSuccess;
+    if (e != cudaSuccess) {
+        delete g;
+        return cuda_fail(e);
+    }
+    *out_capsule = g;
     return ESC_OK;
 }
 

@@ -76,7 +76,9 @@ struct esc_bufset {
     uint64_t layout_digest;
     uint64_t position;                // live: current token position; capsule: boundary P'
     // capsule only
-    uint8_t* slab;
+    uint8_t* slab;                    // device address the copy kernels read (HOST tier: the pinned slab's device alias)
+    uint8_t* slab_host;               // HOST tier: the pinned host address; GPU tier: nullptr
+    uint32_t tier;                    // ESC_TIER_GPU / ESC_TIER_HOST
     uint64_t slab_bytes, payload_bytes, chunk, prefix_digest;
 };
 

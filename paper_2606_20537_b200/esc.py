@@ -24,6 +24,7 @@ SNAPSHOT_ALLOW_UNALIGNED = 1
 MAX_FORK = 16
 MAX_ROWS = 256
 POSITION_UNKNOWN = 2**64 - 1
+TIER_GPU, TIER_HOST = 0, 1
 
 
 class EscError(RuntimeError):
@@ -44,7 +45,7 @@ class BufDesc(C.Structure):
 class CapsuleInfo(C.Structure):
     _fields_ = [("boundary", C.c_uint64), ("chunk", C.c_uint64), ("slab_bytes", C.c_uint64),
                 ("payload_bytes", C.c_uint64), ("layout_digest", C.c_uint64), ("prefix_digest", C.c_uint64),
-                ("n_rows", C.c_uint32), ("n_segments", C.c_uint32), ("aligned", C.c_uint32), ("reserved", C.c_uint32)]
+                ("n_rows", C.c_uint32), ("n_segments", C.c_uint32), ("aligned", C.c_uint32), ("tier", C.c_uint32)]
 
 
 class ScanArgs(C.Structure):
@@ -73,6 +74,8 @@ _sig = {
     "esc_fork": (C.c_int, [_P, C.POINTER(_P), C.c_uint32, _P]),
     "esc_rollback": (C.c_int, [_P, _P, _P]),
     "esc_capsule_info_get": (C.c_int, [_P, C.POINTER(CapsuleInfo)]),
+    "esc_capsule_demote": (C.c_int, [_P, _P, C.c_uint64, _P, C.POINTER(_P)]),
+    "esc_capsule_promote": (C.c_int, [_P, _P, C.c_uint64, _P, C.POINTER(_P)]),
     "esc_capsule_valid_end": (C.c_int, [_P, C.c_uint32, C.POINTER(C.c_uint64)]),
     "esc_shape_key_make": (C.c_uint64, [C.c_uint32] * 7),
     "esc_linattn_scan": (C.c_int, [_P, C.c_uint64] + [_P] * 7 + [C.c_uint64, C.c_uint64, C.c_uint32, _P]),
@@ -217,6 +220,25 @@ def restore(live, capsule, expect_prefix_digest=None, stream=None):
 def fork(capsule, lives, stream=None):
     arr = (_P * len(lives))(*[l.h for l in lives])
     _check(lib.esc_fork(capsule.h, arr, len(lives), _stream(stream)), "esc_fork")
+
+
+def capsule_demote(capsule, storage_host, storage_bytes=None, stream=None):
+    """storage_host: pinned torch uint8 tensor (or host address + storage_bytes). Returns the HOST-tier capsule."""
+    if storage_bytes is None:
+        storage_bytes = storage_host.numel() * storage_host.element_size()
+    h = _P()
+    _check(lib.esc_capsule_demote(capsule.h, _ptr(storage_host), storage_bytes, _stream(stream), C.byref(h)),
+           "esc_capsule_demote")
+    return BufSet(h, keep=(storage_host,))
+
+
+def capsule_promote(host_capsule, storage_dev, storage_bytes=None, stream=None):
+    if storage_bytes is None:
+        storage_bytes = storage_dev.numel() * storage_dev.element_size()
+    h = _P()
+    _check(lib.esc_capsule_promote(host_capsule.h, _ptr(storage_dev), storage_bytes, _stream(stream), C.byref(h)),
+           "esc_capsule_promote")
+    return BufSet(h, keep=(storage_dev,))
 
 
 def rollback(live, capsule_earlier, stream=None):

@@ -204,3 +204,86 @@ def test_full_size_config1_restore_sampled(esc, ctx):
     esc.restore(live.set, cap)
     oracle.capsule_restore(live.oracle_rows(), P, ref)
     live.assert_equals_host()
+
+
+@pytest.mark.parametrize("head_major", [False, True])
+def test_host_tier_demote_restore_promote_bit_exact(esc, ctx, head_major):
+    # SURVEY section 8(f) #2 / PAPER.md:122,125-126,145: tiered handle; promotion = host-backed buffer + async copy.
+    # The host-tier slab holds the oracle's bytes; restore / fork straight from it (zero-copy over the host link) and
+    # promote back to a device slab are byte-exact.
+    P = 448
+    specs = _small_hybrid(512, head_major=head_major)
+    live = LiveSet(esc, ctx, specs, (5, int(head_major)))
+    slab_bytes, payload = live.set.capsule_bytes(P)
+    slab = _slab(slab_bytes)
+    cap = esc.snapshot(live.set, P, 64, slab, prefix_digest=77)
+    host = torch.zeros(slab_bytes, dtype=torch.uint8).pin_memory()
+    hcap = esc.capsule_demote(cap, host)
+    torch.cuda.synchronize()
+    hi = hcap.info()
+    assert hi.tier == esc.TIER_HOST and cap.info().tier == esc.TIER_GPU
+    assert (hi.boundary, hi.payload_bytes, hi.slab_bytes, hi.prefix_digest, hi.layout_digest) == (
+        P, payload, slab_bytes, 77, live.set.layout_digest)
+    ref_slab = _check_snapshot_matches_oracle(live, host, P)       # host slab == oracle's memcpy capsule on valid ranges
+    slab.fill_(0xEE)                                                # the device slab may go away: the host tier is self-contained
+    # restore directly from the host tier after an adversarial dirty
+    live.fill(78, 0, pattern=0xFF)
+    esc.restore(live.set, hcap, expect_prefix_digest=77)
+    oracle.capsule_restore(live.oracle_rows(), P, ref_slab)
+    live.assert_equals_host()
+    assert live.set.position == P
+    # fork from the host tier
+    sessions = [LiveSet(esc, ctx, specs, (5, 10 + i)) for i in range(3)]
+    esc.fork(hcap, [s.set for s in sessions])
+    for s in sessions:
+        oracle.capsule_restore(s.oracle_rows(), P, ref_slab)
+        s.assert_equals_host()
+    # promote into a fresh device slab: a GPU-tier capsule with the same bytes
+    slab2 = _slab(slab_bytes)
+    cap2 = esc.capsule_promote(hcap, slab2)
+    torch.cuda.synchronize()
+    assert cap2.info().tier == esc.TIER_GPU
+    _check_snapshot_matches_oracle(live, slab2, P)
+    live.fill(79, 0)
+    esc.rollback(live.set, cap2)
+    oracle.capsule_restore(live.oracle_rows(), P, ref_slab)
+    live.assert_equals_host()
+    # errors: pageable host memory, wrong tier, short storage — nothing enqueued, no handle returned
+    with pytest.raises(esc.EscError) as e:
+        esc.capsule_demote(cap, torch.zeros(slab_bytes + 256, dtype=torch.uint8)[: slab_bytes])
+    assert e.value.code in (esc.ERR_INVALID, esc.ERR_UNALIGNED)
+    with pytest.raises(esc.EscError) as e:
+        esc.capsule_demote(hcap, host)
+    assert e.value.code == esc.ERR_INVALID
+    with pytest.raises(esc.EscError) as e:
+        esc.capsule_promote(cap, slab2)
+    assert e.value.code == esc.ERR_INVALID
+    with pytest.raises(esc.EscError) as e:
+        esc.capsule_promote(hcap, slab2[: slab_bytes - 256])
+    assert e.value.code == esc.ERR_CAPACITY
+    for c in (cap, hcap, cap2):
+        c.destroy()
+
+
+def test_host_tier_capsule_in_graph(esc, ctx):
+    # the captured restore node reads whatever capsule is bound: binding a HOST-tier capsule needs no recapture either
+    P = 256
+    specs = _small_hybrid(512)
+    live = LiveSet(esc, ctx, specs, (6, 0))
+    slab = _slab(live.set.capsule_bytes(P)[0])
+    cap = esc.snapshot(live.set, P, 64, slab)
+    host = torch.zeros(slab.numel(), dtype=torch.uint8).pin_memory()
+    hcap = esc.capsule_demote(cap, host)
+    torch.cuda.synchronize()
+    ref = oracle.capsule_snapshot(live.oracle_rows(), P)
+    stream = torch.cuda.Stream()
+    graph = esc.graph_capture(ctx, live.set, P, [], stream)
+    for c in (cap, hcap, cap):
+        live.fill(80, 0, pattern=0xFF)
+        torch.cuda.synchronize()
+        graph.set_capsule(c, stream)
+        graph.launch(stream)
+        stream.synchronize()
+        oracle.capsule_restore(live.oracle_rows(), P, ref)
+        live.assert_equals_host()
+    graph.destroy()
