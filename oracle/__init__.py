@@ -10,10 +10,13 @@ What it holds (all pinned by `tests/test_oracle_*.py`, `-m "not gpu"`):
   * linattn_recurrence_np   the same definition restated in numpy (tiny shapes)
   * capsule_*               byte-level memcpy snapshot / restore of a named buffer set
                             (Algorithm 1)
+  * fp8_stage.*             FP8 (E4M3) -> BF16 dequantisation stage (reading 23),
+                            pinned by tests/test_oracle_fp8.py (format closed forms, torch float8_e4m3fn)
 Parity pins: closed form O(T^2), g==1 -> tril(QK^T)V (numpy matmul), scalar IIR
 (scipy.signal.lfilter), hand example, linearity, restore-continue invariant; capsule ->
 memcmp semantics and the size formula.  No function here is "parity unpinned".
 """
+from . import fp8_stage  # noqa: F401
 from .oracle import (  # noqa: F401
     bf16_bits_to_f32,
     linattn_recurrence,
