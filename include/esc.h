@@ -206,6 +206,31 @@ int esc_capsule_demote(const esc_bufset* capsule, void* storage_host, uint64_t s
 int esc_capsule_promote(const esc_bufset* host_capsule, void* storage_dev, uint64_t storage_bytes, void* stream,
                         esc_bufset** out_capsule);
 
+/* ---- FP8 KV rows and their BF16 dequantisation stage (reading 23) -----------
+ * On the long-context route the persistent KV is FP8 and a BF16 working stage is derived from it; the capsule
+ * holds the FP8 bytes only ("FP8-KV roughly halves it") plus the stage's valid end as metadata,
+ * and "the FP8 -> BF16 working stage is rebuilt lazily on the next read, not eagerly in restore".
+ *   attach : declare that live row `row` (a pure per-token row: fixed_bytes == 0) holds FP8 E4M3 codes and has a
+ *            caller-owned BF16 stage of the same shape: stage segment s starts at stage_dev + s * 2 * seg_stride,
+ *            stage element i = bf16_rne(fp32(decode(code_i)) * scale); NaN codes -> 0x7FC0 | sign.  The stage is not
+ *            part of the capsule or of the layout digest.  stage_capacity_bytes >= 2 x the row's capacity.
+ *   valid end: tokens [0, end) of the stage are in sync with the row.  Host-tracked: esc_restore / esc_rollback /
+ *            esc_fork / esc_graph_launch reset it to 0 (the paper's lazy rule); esc_dequant_stage_fill rebuilds
+ *            tokens [end, upto) from the live FP8 row with one kernel launch and sets end = upto; a snapshot
+ *            records the live value in the capsule (readable with the same call on the capsule handle).
+ *   esc_restore_ex(flags = ESC_RESTORE_DEQUANT_EAGER): restore AND rebuild every attached stage over [0, P) in the
+ *            same single kernel launch (each capsule byte is read once and written as FP8 to the row and as BF16 to
+ *            the stage); sets every valid end to P.  flags = 0 is esc_restore. */
+#define ESC_FORMAT_FP8_E4M3 1u
+#define ESC_RESTORE_DEQUANT_EAGER 1u
+#define ESC_ALL_ROWS UINT32_MAX            /* esc_dequant_stage_fill: every row that has a stage, one kernel launch */
+int esc_bufset_attach_dequant_stage(esc_bufset* live, uint32_t row, void* stage_dev, uint64_t stage_capacity_bytes,
+                                    uint32_t format, float scale);
+int esc_dequant_stage_valid_end(const esc_bufset* set, uint32_t row, uint64_t* out_tokens);
+int esc_dequant_stage_fill(esc_bufset* live, uint32_t row, uint64_t upto_tokens, void* stream);
+int esc_restore_ex(esc_bufset* live, const esc_bufset* capsule, const uint64_t* expect_prefix_digest, uint32_t flags,
+                   void* stream);
+
 /* ---- chunked gated linear-attention scan ---------------------------------------------- */
 #define ESC_DTYPE_BF16 1u
 #define ESC_DTYPE_F32  2u

@@ -219,7 +219,10 @@ int esc_snapshot(esc_bufset* live, uint64_t P, uint64_t chunk, uint64_t prefix_d
     cap->ctx = live->ctx;
     cap->frozen = true;
     cap->rows = live->rows;
-    for (Row& r : cap->rows) r.base = nullptr;  // a capsule carries the layout, not the live pointers
+    for (Row& r : cap->rows) {   // a capsule carries the layout (and the stages' valid ends), not the live pointers
+        r.base = nullptr;
+        r.stage = nullptr;
+    }
     cap->layout_digest = live->layout_digest;
     cap->position = P;
     cap->slab = (uint8_t*)storage_dev;
@@ -247,7 +250,7 @@ int esc_snapshot(esc_bufset* live, uint64_t P, uint64_t chunk, uint64_t prefix_d
     return ESC_OK;
 }
 
-static int restore_impl(esc_bufset* live, const esc_bufset* cap, cudaStream_t stream) {
+static int restore_impl(esc_bufset* live, const esc_bufset* cap, cudaStream_t stream, bool eager_dequant = false) {
     std::vector<Seg> segs;
     layout_walk(live->rows, cap->position, &segs, nullptr, nullptr);
     std::vector<const uint8_t*> src(segs.size());
@@ -258,7 +261,24 @@ static int restore_impl(esc_bufset* live, const esc_bufset* cap, cudaStream_t st
         dst[i] = segs[i].live;
         bytes[i] = segs[i].bytes;
     }
-    int rc = launch_copy(live->ctx, src.data(), dst.data(), bytes.data(), (uint32_t)segs.size(), stream);
+    int rc;
+    if (!eager_dequant) {
+        rc = launch_copy(live->ctx, src.data(), dst.data(), bytes.data(), (uint32_t)segs.size(), stream);
+        if (rc == ESC_OK) reset_stage_valid(live, 0);   // "rebuilt lazily on the next read, not eagerly in restore"
+    } else {
+        // same walk order as layout_walk: rows in table order, segments inside a row
+        std::vector<uint8_t*> d16(segs.size(), nullptr);
+        std::vector<float> scale(segs.size(), 1.f);
+        size_t i = 0;
+        for (const Row& r : live->rows)
+            for (uint32_t sg = 0; sg < r.n_seg; ++sg, ++i)
+                if (r.stage) {
+                    d16[i] = r.stage + 2 * ((uint64_t)sg * r.seg_stride);
+                    scale[i] = r.stage_scale;
+                }
+        rc = launch_stage(live->ctx, src.data(), dst.data(), d16.data(), bytes.data(), scale.data(), (uint32_t)segs.size(), stream);
+        if (rc == ESC_OK) reset_stage_valid(live, cap->position);
+    }
     if (rc == ESC_OK) live->position = cap->position;  // "rebind desc"
     return rc;
 }
@@ -268,6 +288,15 @@ int esc_restore(esc_bufset* live, const esc_bufset* capsule, const uint64_t* exp
     if (rc != ESC_OK) return rc;
     if (expect_prefix_digest && *expect_prefix_digest != capsule->prefix_digest) return ESC_ERR_MISMATCH;
     return restore_impl(live, capsule, (cudaStream_t)stream);
+}
+
+int esc_restore_ex(esc_bufset* live, const esc_bufset* capsule, const uint64_t* expect_prefix_digest, uint32_t flags,
+                   void* stream) {
+    if (flags & ~ESC_RESTORE_DEQUANT_EAGER) return ESC_ERR_INVALID;
+    int rc = pair_check(live, capsule);
+    if (rc != ESC_OK) return rc;
+    if (expect_prefix_digest && *expect_prefix_digest != capsule->prefix_digest) return ESC_ERR_MISMATCH;
+    return restore_impl(live, capsule, (cudaStream_t)stream, (flags & ESC_RESTORE_DEQUANT_EAGER) != 0);
 }
 
 int esc_rollback(esc_bufset* live, const esc_bufset* capsule_earlier, void* stream) {
@@ -300,7 +329,10 @@ int esc_fork(const esc_bufset* capsule, esc_bufset* const* lives, uint32_t n, vo
     for (uint32_t d = 0; d < n; ++d) dstp[d] = dst[d].data();
     int rc = launch_fork(capsule->ctx, src.data(), dstp.data(), n, bytes.data(), (uint32_t)ns, (cudaStream_t)stream);
     if (rc == ESC_OK)
-        for (uint32_t d = 0; d < n; ++d) lives[d]->position = capsule->position;
+        for (uint32_t d = 0; d < n; ++d) {
+            lives[d]->position = capsule->position;
+            reset_stage_valid(lives[d], 0);
+        }
     return rc;
 }
 

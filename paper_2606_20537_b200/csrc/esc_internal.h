@@ -59,6 +59,11 @@ struct Row {
     uint8_t* base;
     uint64_t capacity, fixed_bytes, bytes_per_token, seg_stride;
     uint32_t n_seg;
+    // optional BF16 dequantisation stage of an FP8 row (include/esc.h "FP8 KV rows"); not part of the capsule
+    uint8_t* stage = nullptr;
+    uint32_t stage_format = 0;
+    float stage_scale = 1.f;
+    uint64_t stage_valid_tokens = 0;
 };
 
 }  // namespace esc
@@ -106,6 +111,12 @@ int launch_fork(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* c
 // table-in-global-memory variant used inside captured graphs
 void build_copy_table(CopyTable* t, const uint8_t* const* src, uint8_t* const* dst, const uint64_t* bytes, uint32_t n);
 int launch_copy_indirect(const esc_ctx* ctx, const CopyTable* table_dev, uint32_t grid_blocks, cudaStream_t stream);
+
+// staged copy / FP8 -> BF16 expansion (stage.cu): entry i copies bytes[i] from src to dst8 (if not NULL) and writes
+// their BF16 expansion to dst16 (if not NULL)
+int launch_stage(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* dst8, uint8_t* const* dst16,
+                 const uint64_t* bytes, const float* scale, uint32_t n, cudaStream_t stream);
+void reset_stage_valid(esc_bufset* live, uint64_t tokens);
 
 // scan (scan_kernel.cu)
 struct ScanShape {

@@ -139,7 +139,10 @@ int esc_graph_launch(esc_graph* graph, void* stream) {
     if (!graph) return ESC_ERR_INVALID;
     if (graph->live && !graph->bound) return ESC_ERR_INVALID;
     ESC_CUDA(cudaGraphLaunch(graph->exec, (cudaStream_t)stream));
-    if (graph->live) graph->live->position = graph->bound_boundary;
+    if (graph->live) {
+        graph->live->position = graph->bound_boundary;
+        reset_stage_valid(graph->live, 0);   // the restore node copies FP8 rows only: stages are rebuilt lazily
+    }
     return ESC_OK;
 }
 

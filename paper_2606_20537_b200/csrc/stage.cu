@@ -1,0 +1,192 @@
+// FP8 (E4M3) KV rows and their BF16 dequantisation stage (include/esc.h; reading 23).
+//
+// One kernel serves the lazy rebuild (esc_dequant_stage_fill: live FP8 row -> stage) and the eager, fused restore
+// (esc_restore_ex: capsule slab -> live row AND stage, plain rows copied alongside, ONE launch).  Like the capsule
+// copy kernel it is driven by a table of (row, segment) entries cut into 8 KiB tiles of source bytes, one CTA per
+// tile; a thread loads 2 x 16 codes, stores them (when the entry has an FP8 destination) and stores 2 x 32 B of BF16.
+// Roofline: HBM.  Algorithmic bytes per FP8 element: 1 read + 2 written for a fill, 1 + 1 + 2 for a fused restore.
+// Arithmetic per element (the precision both sides take the rounding decisions in): cvt e4m3 -> f16 (exact) -> f32
+// (exact), one fp32 multiply by the row scale, cvt.rn to bf16; NaN codes are replaced by 0x7FC0 | sign.
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_fp8.h>
+#include <string.h>
+
+#include "esc_internal.h"
+
+namespace esc {
+
+constexpr uint32_t kStageMaxSeg = 96;
+constexpr uint32_t kStageTile = kCopyThreads * 2 * 16u;   // 8 KiB of source bytes
+
+struct StageTable {
+    uint32_t n_seg;
+    uint32_t n_tiles;
+    uint32_t tile_begin[kStageMaxSeg + 1];
+    uint32_t pad_;
+    const uint8_t* src[kStageMaxSeg];
+    uint8_t* dst8[kStageMaxSeg];     // FP8 destination (fused restore) or NULL (fill)
+    uint8_t* dst16[kStageMaxSeg];    // BF16 stage or NULL (a plain row copied alongside)
+    uint64_t bytes[kStageMaxSeg];
+    float scale[kStageMaxSeg];
+};
+
+// two E4M3 codes (low byte = element 0) -> two bf16 (low half = element 0)
+__device__ __forceinline__ uint32_t expand2(uint32_t codes, float scale) {
+    const __half2_raw h = __nv_cvt_fp8x2_to_halfraw2((__nv_fp8x2_storage_t)(codes & 0xFFFFu), __NV_E4M3);
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&h));
+    const __nv_bfloat162 b = __floats2bfloat162_rn(f.x * scale, f.y * scale);
+    uint32_t r = *reinterpret_cast<const uint32_t*>(&b);
+    if ((codes & 0x7Fu) == 0x7Fu) r = (r & 0xFFFF0000u) | 0x7FC0u | ((codes & 0x80u) << 8);
+    if ((codes & 0x7F00u) == 0x7F00u) r = (r & 0x0000FFFFu) | ((0x7FC0u | (codes & 0x8000u)) << 16);
+    return r;
+}
+
+__device__ __forceinline__ uint16_t expand1(uint8_t code, float scale) { return (uint16_t)(expand2(code, scale) & 0xFFFFu); }
+
+__global__ void __launch_bounds__(kCopyThreads, 8) esc_stage_kernel(const __grid_constant__ StageTable t) {
+    const uint32_t tid = threadIdx.x;
+    for (uint32_t tile = blockIdx.x; tile < t.n_tiles; tile += gridDim.x) {
+        uint32_t lo = 0, hi = t.n_seg;   // largest e with tile_begin[e] <= tile
+        while (hi - lo > 1) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (t.tile_begin[mid] <= tile) lo = mid;
+            else hi = mid;
+        }
+        const uint32_t e = lo;
+        const uint64_t off = (uint64_t)(tile - t.tile_begin[e]) * kStageTile;
+        const uint64_t left = t.bytes[e] - off;
+        const uint32_t n = (uint32_t)(left < kStageTile ? left : kStageTile);
+        const uint8_t* src = t.src[e] + off;
+        uint8_t* d8 = t.dst8[e] ? t.dst8[e] + off : nullptr;
+        uint8_t* d16 = t.dst16[e] ? t.dst16[e] + 2 * off : nullptr;
+        const float scale = t.scale[e];
+        const bool aligned = ((((uintptr_t)src) | ((uintptr_t)d8) | ((uintptr_t)d16)) & 15u) == 0;
+        uint32_t done = 0;
+        if (aligned) {
+            const uint32_t n16 = n >> 4;
+            for (uint32_t i = tid; i < n16; i += kCopyThreads) {
+                uint4 v;
+                asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                             : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                             : "l"(reinterpret_cast<const uint4*>(src) + i));
+                if (d8) reinterpret_cast<uint4*>(d8)[i] = v;
+                if (d16) {
+                    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+                    uint4 o0, o1;
+                    o0.x = expand2(w[0], scale); o0.y = expand2(w[0] >> 16, scale);
+                    o0.z = expand2(w[1], scale); o0.w = expand2(w[1] >> 16, scale);
+                    o1.x = expand2(w[2], scale); o1.y = expand2(w[2] >> 16, scale);
+                    o1.z = expand2(w[3], scale); o1.w = expand2(w[3] >> 16, scale);
+                    reinterpret_cast<uint4*>(d16)[2 * i] = o0;
+                    reinterpret_cast<uint4*>(d16)[2 * i + 1] = o1;
+                }
+            }
+            done = n16 << 4;
+        }
+        for (uint32_t i = done + tid; i < n; i += kCopyThreads) {   // tails and unaligned pointers: element by element
+            const uint8_t c = src[i];
+            if (d8) d8[i] = c;
+            if (d16) reinterpret_cast<uint16_t*>(d16)[i] = expand1(c, scale);
+        }
+    }
+}
+
+int launch_stage(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* dst8, uint8_t* const* dst16,
+                 const uint64_t* bytes, const float* scale, uint32_t n, cudaStream_t stream) {
+    (void)ctx;
+    for (uint32_t first = 0; first < n; first += kStageMaxSeg) {
+        const uint32_t m = n - first < kStageMaxSeg ? n - first : kStageMaxSeg;
+        StageTable t;
+        memset(&t, 0, sizeof t);
+        t.n_seg = m;
+        uint64_t tiles = 0;
+        for (uint32_t i = 0; i < m; ++i) {
+            t.tile_begin[i] = (uint32_t)tiles;
+            tiles += (bytes[first + i] + kStageTile - 1) / kStageTile;
+            t.src[i] = src[first + i];
+            t.dst8[i] = dst8[first + i];
+            t.dst16[i] = dst16[first + i];
+            t.bytes[i] = bytes[first + i];
+            t.scale[i] = scale[first + i];
+        }
+        t.tile_begin[m] = (uint32_t)tiles;
+        t.n_tiles = (uint32_t)tiles;
+        if (tiles == 0) continue;
+        esc_stage_kernel<<<copy_grid_blocks(tiles), kCopyThreads, 0, stream>>>(t);
+        ESC_CUDA(cudaGetLastError());
+    }
+    return ESC_OK;
+}
+
+void reset_stage_valid(esc_bufset* live, uint64_t tokens) {
+    for (Row& r : live->rows)
+        if (r.stage) r.stage_valid_tokens = tokens;
+}
+
+}  // namespace esc
+
+using namespace esc;
+
+extern "C" {
+
+int esc_bufset_attach_dequant_stage(esc_bufset* live, uint32_t row, void* stage_dev, uint64_t stage_capacity_bytes,
+                                    uint32_t format, float scale) {
+    if (!live || live->frozen || row >= live->rows.size() || !stage_dev) return ESC_ERR_INVALID;
+    if (format != ESC_FORMAT_FP8_E4M3) return ESC_ERR_UNSUPPORTED;
+    Row& r = live->rows[row];
+    if (r.fixed_bytes != 0 || r.bytes_per_token == 0) return ESC_ERR_INVALID;   // a pure per-token (KV) row
+    if (!(scale == scale) || scale == 0.f) return ESC_ERR_INVALID;
+    if (stage_capacity_bytes / 2 < r.capacity) return ESC_ERR_CAPACITY;
+    if ((uintptr_t)stage_dev & 1u) return ESC_ERR_UNALIGNED;
+    r.stage = (uint8_t*)stage_dev;
+    r.stage_format = format;
+    r.stage_scale = scale;
+    r.stage_valid_tokens = 0;
+    return ESC_OK;
+}
+
+int esc_dequant_stage_valid_end(const esc_bufset* set, uint32_t row, uint64_t* out_tokens) {
+    if (!set || !out_tokens || row >= set->rows.size()) return ESC_ERR_INVALID;
+    if (!set->rows[row].stage_format) return ESC_ERR_INVALID;
+    *out_tokens = set->rows[row].stage_valid_tokens;
+    return ESC_OK;
+}
+
+int esc_dequant_stage_fill(esc_bufset* live, uint32_t row, uint64_t upto_tokens, void* stream) {
+    if (!live || live->frozen || (row != ESC_ALL_ROWS && row >= live->rows.size())) return ESC_ERR_INVALID;
+    if (live->position != ESC_POSITION_UNKNOWN && upto_tokens > live->position) return ESC_ERR_MISMATCH;
+    std::vector<Row*> todo;
+    for (size_t i = 0; i < live->rows.size(); ++i)
+        if ((row == ESC_ALL_ROWS || row == i) && live->rows[i].stage) todo.push_back(&live->rows[i]);
+    if (todo.empty()) return ESC_ERR_INVALID;   // no stage attached
+    for (Row* r : todo) {
+        std::vector<Row> one(1, *r);
+        int rc = check_fit(one, upto_tokens);
+        if (rc != ESC_OK) return rc;
+    }
+    std::vector<const uint8_t*> src;
+    std::vector<uint8_t*> d8, d16;
+    std::vector<uint64_t> bytes;
+    std::vector<float> scale;
+    for (Row* r : todo) {
+        const uint64_t from = r->stage_valid_tokens;
+        if (upto_tokens <= from) continue;   // already in sync
+        for (uint32_t s = 0; s < r->n_seg; ++s) {
+            src.push_back(r->base + (uint64_t)s * r->seg_stride + from * r->bytes_per_token);
+            d8.push_back(nullptr);
+            d16.push_back(r->stage + 2 * ((uint64_t)s * r->seg_stride + from * r->bytes_per_token));
+            bytes.push_back((upto_tokens - from) * r->bytes_per_token);
+            scale.push_back(r->stage_scale);
+        }
+    }
+    if (src.empty()) return ESC_OK;
+    int rc = launch_stage(live->ctx, src.data(), d8.data(), d16.data(), bytes.data(), scale.data(), (uint32_t)src.size(),
+                          (cudaStream_t)stream);
+    if (rc == ESC_OK)
+        for (Row* r : todo)
+            if (r->stage_valid_tokens < upto_tokens) r->stage_valid_tokens = upto_tokens;
+    return rc;
+}
+
+}  // extern "C"

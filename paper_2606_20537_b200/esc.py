@@ -25,6 +25,9 @@ MAX_FORK = 16
 MAX_ROWS = 256
 POSITION_UNKNOWN = 2**64 - 1
 TIER_GPU, TIER_HOST = 0, 1
+FORMAT_FP8_E4M3 = 1
+ALL_ROWS = 2**32 - 1
+RESTORE_DEQUANT_EAGER = 1
 
 
 class EscError(RuntimeError):
@@ -76,6 +79,10 @@ _sig = {
     "esc_capsule_info_get": (C.c_int, [_P, C.POINTER(CapsuleInfo)]),
     "esc_capsule_demote": (C.c_int, [_P, _P, C.c_uint64, _P, C.POINTER(_P)]),
     "esc_capsule_promote": (C.c_int, [_P, _P, C.c_uint64, _P, C.POINTER(_P)]),
+    "esc_bufset_attach_dequant_stage": (C.c_int, [_P, C.c_uint32, _P, C.c_uint64, C.c_uint32, C.c_float]),
+    "esc_dequant_stage_valid_end": (C.c_int, [_P, C.c_uint32, C.POINTER(C.c_uint64)]),
+    "esc_dequant_stage_fill": (C.c_int, [_P, C.c_uint32, C.c_uint64, _P]),
+    "esc_restore_ex": (C.c_int, [_P, _P, C.POINTER(C.c_uint64), C.c_uint32, _P]),
     "esc_capsule_valid_end": (C.c_int, [_P, C.c_uint32, C.POINTER(C.c_uint64)]),
     "esc_shape_key_make": (C.c_uint64, [C.c_uint32] * 7),
     "esc_linattn_scan": (C.c_int, [_P, C.c_uint64] + [_P] * 7 + [C.c_uint64, C.c_uint64, C.c_uint32, _P]),
@@ -184,6 +191,22 @@ class BufSet:
         _check(lib.esc_capsule_valid_end(self.h, row, C.byref(n)), "esc_capsule_valid_end")
         return n.value
 
+    def attach_dequant_stage(self, row, stage, scale=1.0, fmt=FORMAT_FP8_E4M3, stage_bytes=None):
+        """stage: torch bf16/uint8 tensor (or device address + stage_bytes) shaped like the FP8 row, 2 bytes per code."""
+        if stage_bytes is None:
+            stage_bytes = stage.numel() * stage.element_size()
+        _check(lib.esc_bufset_attach_dequant_stage(self.h, row, _ptr(stage), stage_bytes, fmt, scale),
+               "esc_bufset_attach_dequant_stage")
+        self._keep = tuple(self._keep) + (stage,)
+
+    def stage_valid_end(self, row):
+        n = C.c_uint64()
+        _check(lib.esc_dequant_stage_valid_end(self.h, row, C.byref(n)), "esc_dequant_stage_valid_end")
+        return n.value
+
+    def stage_fill(self, row, upto_tokens, stream=None):
+        _check(lib.esc_dequant_stage_fill(self.h, row, upto_tokens, _stream(stream)), "esc_dequant_stage_fill")
+
     def destroy(self):
         if self.h:
             lib.esc_bufset_destroy(self.h)
@@ -215,6 +238,11 @@ def snapshot(live, P, chunk, storage, storage_bytes=None, prefix_digest=0, flags
 def restore(live, capsule, expect_prefix_digest=None, stream=None):
     e = None if expect_prefix_digest is None else C.byref(C.c_uint64(expect_prefix_digest))
     _check(lib.esc_restore(live.h, capsule.h, e, _stream(stream)), "esc_restore")
+
+
+def restore_ex(live, capsule, expect_prefix_digest=None, flags=0, stream=None):
+    e = None if expect_prefix_digest is None else C.byref(C.c_uint64(expect_prefix_digest))
+    _check(lib.esc_restore_ex(live.h, capsule.h, e, flags, _stream(stream)), "esc_restore_ex")
 
 
 def fork(capsule, lives, stream=None):
