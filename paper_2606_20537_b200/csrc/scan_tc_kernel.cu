@@ -66,9 +66,14 @@ constexpr int kVtThreads = 128;   // threads of the four V~ warps
 
 #ifdef ESC_TC_TRACE   // bring-up only: per-chunk clock64() stamps of CTA (0,0), read back with esc_debug_trace_read
 __device__ long long g_tc_trace[16 * 64];
+__device__ unsigned int g_tc_launch;
 #define TC_TRACE(ev, c) do { if (blockIdx.x == 0 && blockIdx.y == 0 && (c) < 64) g_tc_trace[(ev) * 64 + (c)] = clock64(); } while (0)
+// launch-level stamps (globaltimer, ns) of CTA (0,0) thread 0, one column per launch
+__device__ __forceinline__ long long tc_gtime() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define TC_TRACE_L(ev, id) do { if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) g_tc_trace[(ev) * 64 + ((id) & 63)] = tc_gtime(); } while (0)
 #else
 #define TC_TRACE(ev, c) do { } while (0)
+#define TC_TRACE_L(ev, id) do { } while (0)
 #endif
 
 template <int DK, int C>
@@ -203,6 +208,11 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     const uint32_t n_chunks = (uint32_t)((T + C - 1) / C);
     const int q = warp & 3;   // TMEM lane quadrant this warp may access
     if (threadIdx.x == 0) TC_TRACE(9, 0);
+#ifdef ESC_TC_TRACE
+    unsigned int launch_id = 0;
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) launch_id = atomicAdd(&g_tc_launch, 1u);
+    TC_TRACE_L(13, launch_id);
+#endif
     // Programmatic dependent launch: the next kernel of the stream / graph (typically the next layer's scan) may start
     // its on-chip setup while this one runs; everything this kernel reads from or writes to global memory comes after
     // griddepcontrol.wait below, i.e. after the preceding kernel has completed and flushed.
@@ -262,6 +272,9 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     tc_fence_after_sync();
     const uint32_t tb = *tmem_slot;
     asm volatile("griddepcontrol.wait;" ::: "memory");   // ---- global memory may be touched from here on ----
+#ifdef ESC_TC_TRACE
+    TC_TRACE_L(14, launch_id);
+#endif
     if (threadIdx.x == 0) TC_TRACE(10, 0);
 
     // state warps own the carry: row `krow` of the [d_k x 16] slice per thread, fp32 registers
@@ -660,8 +673,11 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     // and no peer still multicasts, copies or arrives into this CTA once the whole cluster is here ----
     tc_fence_before_sync();
     if (threadIdx.x == 0) TC_TRACE(11, 0);
-    cluster_sync();
+    cluster_sync_relaxed();
     if (threadIdx.x == 0) TC_TRACE(12, 0);
+#ifdef ESC_TC_TRACE
+    TC_TRACE_L(15, launch_id);
+#endif
     if (warp == 2) tmem_dealloc(tb, L::tmem_cols);
 }
 

@@ -83,6 +83,12 @@ __device__ __forceinline__ void cluster_sync() {
     asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
     asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+// execution barrier only (no memory ordering): teardown — nobody reads a peer's memory afterwards, and a .release arrive
+// would first wait for this thread's outstanding global stores (measured: ~0.9 us at the end of every launch)
+__device__ __forceinline__ void cluster_sync_relaxed() {
+    asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.aligned;" ::: "memory");
+}
 // shared::cta address of this CTA -> shared::cluster address of the same offset in CTA `rank`
 __device__ __forceinline__ uint32_t mapa(uint32_t cta_addr, uint32_t rank) {
     uint32_t r;
