@@ -294,6 +294,27 @@ int esc_graph_set_capsule(esc_graph* graph, const esc_bufset* capsule, void* str
 int esc_graph_launch(esc_graph* graph, void* stream);
 int esc_graph_destroy(esc_graph* graph);
 
+/* ---- Graph[key] table ("replay Graph[key]"; "a bounded set of shape variants
+ * (the ShapeKey table with LRU eviction) and a fixed maximum sequence length") -------------------------------------
+ * Mechanism only: a bounded map  plan key -> captured esc_graph  kept in the context, least-recently-used eviction.
+ * Which suffix lengths / boundaries get a bucket is the caller's policy; the helpers below give the usual choice.
+ *   esc_suffix_bucket(T, chunk): the smallest chunk * 2^k >= T (0 for T == 0).  A plan captured for the bucket serves
+ *       any suffix T' <= bucket whose tail the caller pads with k = v = 0, g = 1 tokens (reading 13: the state
+ *       and the real tokens' outputs are bit-identical to a T'-token scan, the chunk grid being the same).
+ *   esc_plan_key_make(shape key, suffix bucket, max boundary, n_layers): opaque 64-bit key (FNV-1a of the four).
+ *   put: the table takes ownership of `graph`; inserting into a full table destroys the least recently used plan;
+ *        putting an existing key replaces (and destroys) the old plan.  capacity >= 1 (default 8).
+ *   get: ESC_OK and the plan (now most recently used), or ESC_ERR_MISMATCH when the key is absent — "a new shape
+ *        needing capture": the caller captures and puts.  The table still owns the plan.
+ *   stats: hits, misses, evictions since the context was created. */
+uint64_t esc_suffix_bucket(uint64_t T, uint64_t chunk);
+uint64_t esc_plan_key_make(esc_shape_key key, uint64_t suffix_bucket, uint64_t max_boundary, uint32_t n_layers);
+int esc_plan_table_set_capacity(esc_ctx* ctx, uint32_t capacity);
+int esc_plan_table_put(esc_ctx* ctx, uint64_t plan_key, esc_graph* graph);
+int esc_plan_table_get(esc_ctx* ctx, uint64_t plan_key, esc_graph** out_graph);
+int esc_plan_table_stats(const esc_ctx* ctx, uint32_t* out_size, uint64_t* out_hits, uint64_t* out_misses,
+                         uint64_t* out_evictions);
+
 #ifdef __cplusplus
 }
 #endif

@@ -8,6 +8,7 @@
 
 namespace esc {
 
+void free_plan_table(esc_ctx* ctx);   // graph.cu
 thread_local int g_last_cuda_error = 0;
 
 static inline uint64_t up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
@@ -114,6 +115,7 @@ int esc_ctx_create(int device, esc_ctx** out_ctx) {
 
 int esc_ctx_destroy(esc_ctx* ctx) {
     if (!ctx) return ESC_ERR_INVALID;
+    free_plan_table(ctx);   // the Graph[key] table owns its plans
     delete ctx;
     return ESC_OK;
 }

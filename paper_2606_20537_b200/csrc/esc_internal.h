@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "esc.h"
@@ -68,10 +69,15 @@ struct Row {
 
 }  // namespace esc
 
+struct esc_graph;
 struct esc_ctx {
     int device;
     int sm_count;
     int l2_bytes;
+    // Graph[key] table (include/esc.h): most recently used first
+    std::vector<std::pair<uint64_t, esc_graph*>> plans;
+    uint32_t plan_capacity = 8;
+    uint64_t plan_hits = 0, plan_misses = 0, plan_evictions = 0;
 };
 
 struct esc_bufset {

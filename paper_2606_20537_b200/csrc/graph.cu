@@ -22,6 +22,14 @@ struct esc_graph {
 
 using namespace esc;
 
+static void graph_free(esc_graph* g);
+namespace esc {
+void free_plan_table(esc_ctx* ctx) {
+    for (auto& e : ctx->plans) graph_free(e.second);
+    ctx->plans.clear();
+}
+}  // namespace esc
+
 static void graph_free(esc_graph* g) {
     if (!g) return;
     if (g->exec) cudaGraphExecDestroy(g->exec);
@@ -149,6 +157,80 @@ int esc_graph_launch(esc_graph* graph, void* stream) {
 int esc_graph_destroy(esc_graph* graph) {
     if (!graph) return ESC_ERR_INVALID;
     graph_free(graph);
+    return ESC_OK;
+}
+
+// ---- Graph[key] table: bounded, LRU ------------------------------------------------
+uint64_t esc_suffix_bucket(uint64_t T, uint64_t chunk) {
+    if (T == 0 || chunk == 0) return T;
+    uint64_t b = chunk;
+    while (b < T && b <= (UINT64_MAX >> 1)) b <<= 1;
+    return b;
+}
+
+uint64_t esc_plan_key_make(esc_shape_key key, uint64_t suffix_bucket, uint64_t max_boundary, uint32_t n_layers) {
+    uint64_t h = 0xcbf29ce484222325ull;
+    const uint64_t v[4] = {key, suffix_bucket, max_boundary, n_layers};
+    const uint8_t* b = (const uint8_t*)v;
+    for (size_t i = 0; i < sizeof v; ++i) {
+        h ^= b[i];
+        h *= 0x100000001b3ull;
+    }
+    return h;
+}
+
+static void plan_evict_to(esc_ctx* ctx, size_t n) {
+    while (ctx->plans.size() > n) {
+        graph_free(ctx->plans.back().second);
+        ctx->plans.pop_back();
+        ++ctx->plan_evictions;
+    }
+}
+
+int esc_plan_table_set_capacity(esc_ctx* ctx, uint32_t capacity) {
+    if (!ctx || capacity == 0) return ESC_ERR_INVALID;
+    ctx->plan_capacity = capacity;
+    plan_evict_to(ctx, capacity);
+    return ESC_OK;
+}
+
+int esc_plan_table_put(esc_ctx* ctx, uint64_t plan_key, esc_graph* graph) {
+    if (!ctx || !graph || graph->ctx != ctx) return ESC_ERR_INVALID;
+    for (size_t i = 0; i < ctx->plans.size(); ++i) {
+        if (ctx->plans[i].second == graph && ctx->plans[i].first != plan_key) return ESC_ERR_INVALID;   // already owned under another key
+        if (ctx->plans[i].first == plan_key) {
+            if (ctx->plans[i].second != graph) graph_free(ctx->plans[i].second);
+            ctx->plans.erase(ctx->plans.begin() + i);
+            break;
+        }
+    }
+    plan_evict_to(ctx, ctx->plan_capacity - 1);
+    ctx->plans.insert(ctx->plans.begin(), std::make_pair(plan_key, graph));
+    return ESC_OK;
+}
+
+int esc_plan_table_get(esc_ctx* ctx, uint64_t plan_key, esc_graph** out_graph) {
+    if (!ctx || !out_graph) return ESC_ERR_INVALID;
+    for (size_t i = 0; i < ctx->plans.size(); ++i)
+        if (ctx->plans[i].first == plan_key) {
+            std::pair<uint64_t, esc_graph*> e = ctx->plans[i];
+            ctx->plans.erase(ctx->plans.begin() + i);
+            ctx->plans.insert(ctx->plans.begin(), e);
+            ++ctx->plan_hits;
+            *out_graph = e.second;
+            return ESC_OK;
+        }
+    ++ctx->plan_misses;
+    return ESC_ERR_MISMATCH;
+}
+
+int esc_plan_table_stats(const esc_ctx* ctx, uint32_t* out_size, uint64_t* out_hits, uint64_t* out_misses,
+                         uint64_t* out_evictions) {
+    if (!ctx) return ESC_ERR_INVALID;
+    if (out_size) *out_size = (uint32_t)ctx->plans.size();
+    if (out_hits) *out_hits = ctx->plan_hits;
+    if (out_misses) *out_misses = ctx->plan_misses;
+    if (out_evictions) *out_evictions = ctx->plan_evictions;
     return ESC_OK;
 }
 

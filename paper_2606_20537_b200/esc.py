@@ -90,6 +90,13 @@ _sig = {
     "esc_graph_set_capsule": (C.c_int, [_P, _P, _P]),
     "esc_graph_launch": (C.c_int, [_P, _P]),
     "esc_graph_destroy": (C.c_int, [_P]),
+    "esc_suffix_bucket": (C.c_uint64, [C.c_uint64, C.c_uint64]),
+    "esc_plan_key_make": (C.c_uint64, [C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32]),
+    "esc_plan_table_set_capacity": (C.c_int, [_P, C.c_uint32]),
+    "esc_plan_table_put": (C.c_int, [_P, C.c_uint64, _P]),
+    "esc_plan_table_get": (C.c_int, [_P, C.c_uint64, C.POINTER(_P)]),
+    "esc_plan_table_stats": (C.c_int, [_P, C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64),
+                                       C.POINTER(C.c_uint64)]),
 }
 for _n, (_r, _a) in _sig.items():
     _f = getattr(lib, _n)
@@ -147,6 +154,31 @@ class Ctx:
         n = C.c_int()
         _check(lib.esc_ctx_sm_count(self.h, C.byref(n)), "esc_ctx_sm_count")
         return n.value
+
+    # Graph[key] table (bounded, LRU): the context owns the plans put into it
+    def plan_table_set_capacity(self, n):
+        _check(lib.esc_plan_table_set_capacity(self.h, n), "esc_plan_table_set_capacity")
+
+    def plan_put(self, plan_key, graph):
+        _check(lib.esc_plan_table_put(self.h, plan_key, graph.h), "esc_plan_table_put")
+        graph.owned = False
+        self._plans = getattr(self, "_plans", {})
+        self._plans[plan_key] = graph   # keeps the python references (buffers) of the plan alive
+
+    def plan_get(self, plan_key):
+        """The captured plan or None ("a new shape needing capture")."""
+        h = _P()
+        rc = lib.esc_plan_table_get(self.h, plan_key, C.byref(h))
+        if rc == ERR_MISMATCH:
+            return None
+        _check(rc, "esc_plan_table_get")
+        g = getattr(self, "_plans", {}).get(plan_key)
+        return g if g is not None and g.h and g.h.value == h.value else Graph(h, owned=False)
+
+    def plan_stats(self):
+        n, a, b, c = C.c_uint32(), C.c_uint64(), C.c_uint64(), C.c_uint64()
+        _check(lib.esc_plan_table_stats(self.h, C.byref(n), C.byref(a), C.byref(b), C.byref(c)), "esc_plan_table_stats")
+        return {"size": n.value, "hits": a.value, "misses": b.value, "evictions": c.value}
 
     def close(self):
         if self.h:
@@ -283,10 +315,19 @@ def scan_args(key, q, k, v, g, state_in, state_out, o, T, t_stride, chunk):
                     T, t_stride, chunk, 0)
 
 
+def suffix_bucket(T, chunk):
+    return int(lib.esc_suffix_bucket(T, chunk))
+
+
+def plan_key_make(shape_key, bucket, max_boundary, n_layers):
+    return int(lib.esc_plan_key_make(shape_key, bucket, max_boundary, n_layers))
+
+
 class Graph:
-    def __init__(self, handle, keep=()):
+    def __init__(self, handle, keep=(), owned=True):
         self.h = handle
         self._keep = keep
+        self.owned = owned      # False once a context's plan table owns the handle
 
     def set_capsule(self, capsule, stream=None):
         _check(lib.esc_graph_set_capsule(self.h, capsule.h, _stream(stream)), "esc_graph_set_capsule")
@@ -295,9 +336,9 @@ class Graph:
         _check(lib.esc_graph_launch(self.h, _stream(stream)), "esc_graph_launch")
 
     def destroy(self):
-        if self.h:
+        if self.h and self.owned:
             lib.esc_graph_destroy(self.h)
-            self.h = None
+        self.h = None
 
 
 def graph_capture(ctx, live, max_boundary, layers, stream):

@@ -87,3 +87,14 @@ def test_product_never_imports_oracle():
                 txt = open(os.path.join(dp, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
                 assert "oracle/" not in txt and "_oracle.so" not in txt, f
+
+
+def test_suffix_bucket_and_plan_key(esc):
+    # the smallest chunk * 2^k >= T ("the suffix falls within a captured shape bucket")
+    assert [esc.suffix_bucket(t, 64) for t in (0, 1, 64, 65, 128, 129, 1000, 4096)] == [0, 64, 64, 128, 128, 256, 1024, 4096]
+    assert esc.suffix_bucket(100, 128) == 128 and esc.suffix_bucket(7, 0) == 7
+    k = esc.shape_key_make(1, 16, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, 64)
+    keys = {esc.plan_key_make(k, b, P, n) for b in (64, 128) for P in (2048, 4096) for n in (1, 18)}
+    assert len(keys) == 8 and esc.plan_key_make(k, 64, 2048, 18) in keys
+    assert esc.lib.esc_plan_table_get(None, 1, None) == esc.ERR_INVALID
+    assert esc.lib.esc_plan_table_set_capacity(None, 4) == esc.ERR_INVALID

@@ -181,3 +181,47 @@ def test_config3_fork_continue_rollback_replay(esc, ctx):
     o_ref, s_ref = oracle.linattn_recurrence(qf, kf, vf, gf, src.states[5].cpu().numpy().astype(np.float64))
     assert err_o(inputs[3].out[5].cpu().numpy(), o_ref) <= TOL_O
     assert err_s(second[3][0][5].cpu().numpy(), s_ref) <= TOL_S
+
+
+def test_plan_table_lru_and_padded_bucket(esc):
+    # SURVEY 8(f) #4 / PAPER.md:195,386: bounded Graph[key] table with LRU eviction; a plan captured for a suffix bucket
+    # serves a shorter suffix padded with k = v = 0, g = 1 tokens, bit-identically to the unpadded scan.
+    ctx = esc.Ctx(0)
+    stream = torch.cuda.Stream()
+    b_, h_, chunk = 1, 2, 64
+    key = esc.shape_key_make(b_, h_, DK, DV, esc.DTYPE_BF16, esc.DTYPE_F32, chunk)
+    T = 100
+    bucket = esc.suffix_bucket(T, chunk)
+    assert bucket == 128
+    si = synth.scan_inputs(b_, T, h_, DK, DV, seed_ids=(50,), gate="slow")
+    q, k, v, g = scan_dev_inputs(si)
+    pad = lambda x, val: torch.cat([x, torch.full((b_, bucket - T) + tuple(x.shape[2:]), val, dtype=x.dtype, device=DEV)], dim=1).contiguous()
+    qp, kp, vp, gp = pad(q, 1.0), pad(k, 0.0), pad(v, 0.0), pad(g, 1.0)
+    s0 = torch.from_numpy(synth.scan_state(b_, h_, DK, DV, seed_ids=(51,), scale=0.3)).to(DEV)
+    # reference: the unpadded T-token scan
+    s_ref, o_ref = s0.clone(), torch.zeros((b_, T, h_, DV), dtype=torch.float32, device=DEV)
+    esc.linattn_scan(ctx, key, q, k, v, g, s_ref, s_ref, o_ref, T, T, chunk)
+    state = s0.clone()
+    o = torch.zeros((b_, bucket, h_, DV), dtype=torch.float32, device=DEV)
+
+    def capture(n):
+        return esc.graph_capture(ctx, None, 0, [esc.scan_args(key, qp, kp, vp, gp, state, state, o, bucket, bucket, chunk)] * n, stream)
+
+    ctx.plan_table_set_capacity(2)
+    pk = [esc.plan_key_make(key, bucket, 0, n) for n in (1, 2, 3)]
+    assert ctx.plan_get(pk[0]) is None                       # a new shape needing capture
+    ctx.plan_put(pk[0], capture(1))
+    ctx.plan_put(pk[1], capture(2))
+    plan = ctx.plan_get(pk[0])                               # hit; pk[0] becomes most recently used
+    assert plan is not None
+    plan.launch(stream)
+    stream.synchronize()
+    assert bits_equal(o[:, :T], o_ref) and bits_equal(state, s_ref)
+    ctx.plan_put(pk[2], capture(3))                          # table full: evicts the least recently used = pk[1]
+    assert ctx.plan_get(pk[1]) is None and ctx.plan_get(pk[0]) is not None and ctx.plan_get(pk[2]) is not None
+    st = ctx.plan_stats()
+    assert st == {"size": 2, "hits": 3, "misses": 2, "evictions": 1}
+    ctx.plan_table_set_capacity(1)                           # shrinking evicts down to the most recently used (pk[2])
+    assert ctx.plan_get(pk[0]) is None and ctx.plan_get(pk[2]) is not None
+    assert ctx.plan_stats()["evictions"] == 2
+    ctx.close()                                              # the context destroys the plans it still owns
