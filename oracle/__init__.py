@@ -12,6 +12,8 @@ What it holds (all pinned by `tests/test_oracle_*.py`, `-m "not gpu"`):
                             (Algorithm 1)
   * fp8_stage.*             FP8 (E4M3) -> BF16 dequantisation stage (reading 23),
                             pinned by tests/test_oracle_fp8.py (format closed forms, torch float8_e4m3fn)
+  * gdn_recurrence / causal_conv   gated delta rule and short causal convolution with carried window (the paper's
+                            model family; reading 25), pinned by tests/test_oracle_gdn.py
 Parity pins: closed form O(T^2), g==1 -> tril(QK^T)V (numpy matmul), scalar IIR
 (scipy.signal.lfilter), hand example, linearity, restore-continue invariant; capsule ->
 memcmp semantics and the size formula.  No function here is "parity unpinned".
@@ -21,6 +23,8 @@ from .oracle import (  # noqa: F401
     bf16_bits_to_f32,
     linattn_recurrence,
     linattn_recurrence_np,
+    gdn_recurrence,
+    causal_conv,
     CapsuleRow,
     capsule_payload_bytes,
     capsule_slab_bytes,

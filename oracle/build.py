@@ -8,7 +8,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["linattn_oracle.c", "capsule_oracle.c"]
+SOURCES = ["linattn_oracle.c", "capsule_oracle.c", "gdn_oracle.c"]
 TARGET = os.path.join(HERE, "_oracle.so")
 
 
@@ -24,7 +24,7 @@ def build(force: bool = False) -> str:
         return TARGET
     tmp = TARGET + ".tmp.%d" % os.getpid()
     cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-Wall", "-Wextra",
-           "-o", tmp] + [os.path.join(HERE, s) for s in SOURCES]
+           "-o", tmp] + [os.path.join(HERE, s) for s in SOURCES] + ["-lm"]
     subprocess.run(cmd, check=True)
     os.replace(tmp, TARGET)
     return TARGET

@@ -20,6 +20,10 @@ def _load():
         lib = C.CDLL(path)
         lib.esc_oracle_linattn.restype = C.c_int
         lib.esc_oracle_linattn.argtypes = [C.c_void_p] * 7 + [C.c_int64] * 6 + [C.c_int]
+        lib.esc_oracle_gdn.restype = C.c_int
+        lib.esc_oracle_gdn.argtypes = [C.c_void_p] * 8 + [C.c_int64] * 6 + [C.c_int]
+        lib.esc_oracle_causal_conv.restype = C.c_int
+        lib.esc_oracle_causal_conv.argtypes = [C.c_void_p] * 5 + [C.c_int64] * 5 + [C.c_int]
         lib.esc_oracle_max_threads.restype = C.c_int
         for name in ("esc_oracle_capsule_payload_bytes", "esc_oracle_capsule_slab_bytes"):
             f = getattr(lib, name)
@@ -81,6 +85,51 @@ def linattn_recurrence(q, k, v, g, state_in=None, T=None, n_threads=0):
     if rc != 0:
         raise RuntimeError("esc_oracle_linattn failed rc=%d" % rc)
     return o, s_out
+
+
+def gdn_recurrence(q, k, v, g, beta, state_in=None, T=None, n_threads=0):
+    """fp64 sequential gated delta rule (C; oracle/gdn_oracle.c, reading 25).  Shapes as linattn_recurrence,
+    beta like g.  Returns (o float64 [B,T,H,dv], state_out float64 [B,H,dk,dv])."""
+    q, k, v, g, beta = (np.ascontiguousarray(a, dtype=np.float32) for a in (q, k, v, g, beta))
+    B, Tbuf, H, dk = q.shape
+    dv = v.shape[-1]
+    T = Tbuf if T is None else T
+    assert k.shape == q.shape and v.shape == (B, Tbuf, H, dv) and g.shape == (B, Tbuf, H) == beta.shape and 0 <= T <= Tbuf
+    o = np.empty((B, T, H, dv), dtype=np.float64)
+    s_out = np.empty((B, H, dk, dv), dtype=np.float64)
+    s_in_p = None
+    if state_in is not None:
+        s_in = np.ascontiguousarray(state_in, dtype=np.float64)
+        assert s_in.shape == (B, H, dk, dv)
+        s_in_p = s_in.ctypes.data
+    rc = _load().esc_oracle_gdn(q.ctypes.data, k.ctypes.data, v.ctypes.data, g.ctypes.data, beta.ctypes.data, s_in_p,
+                                o.ctypes.data, s_out.ctypes.data, B, T, Tbuf, H, dk, dv, int(n_threads))
+    if rc != 0:
+        raise RuntimeError("esc_oracle_gdn failed rc=%d" % rc)
+    return o, s_out
+
+
+def causal_conv(x, w, state_in=None, T=None, silu=False):
+    """fp64 short causal depthwise convolution with carried window (C; oracle/gdn_oracle.c).
+    x float32 [B,Tbuf,C]; w float32 [C,W]; state [B,C,W-1] (oldest first).  Returns (y [B,T,C], state_out [B,C,W-1])."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    w = np.ascontiguousarray(w, dtype=np.float32)
+    B, Tbuf, Cc = x.shape
+    W = w.shape[1]
+    T = Tbuf if T is None else T
+    assert w.shape[0] == Cc and 0 <= T <= Tbuf
+    y = np.empty((B, T, Cc), dtype=np.float64)
+    s_out = np.empty((B, Cc, max(W - 1, 0)), dtype=np.float64)
+    s_in_p = None
+    if state_in is not None:
+        s_in = np.ascontiguousarray(state_in, dtype=np.float64)
+        assert s_in.shape == (B, Cc, W - 1)
+        s_in_p = s_in.ctypes.data
+    rc = _load().esc_oracle_causal_conv(x.ctypes.data, w.ctypes.data, s_in_p, y.ctypes.data, s_out.ctypes.data,
+                                        B, T, Tbuf, Cc, W, int(bool(silu)))
+    if rc != 0:
+        raise RuntimeError("esc_oracle_causal_conv failed rc=%d" % rc)
+    return y, s_out
 
 
 def linattn_recurrence_np(q, k, v, g, state_in=None):
