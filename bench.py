@@ -481,6 +481,30 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
     cap8.destroy()
     live8.destroy()
     del bufs8, stages8, slab8
+    # ---- gated delta rule + convolution state, v0 kernels: one layer at config 2's cold length ----
+    Tg = 16384 + SUFFIX
+    gin = workload.SuffixInputs(1, Tg, seed=11, device=dev)
+    beta = torch.from_numpy(synth.gdn_beta(workload.B, Tg, workload.H, seed_ids=(11,))).to(dev)
+    gstate = torch.zeros((workload.B, workload.H, 128, 128), dtype=torch.float32, device=dev)
+    gq, gk, gv, gg = gin.dev[0]
+    gdn_ms, _ = med_ms(lambda: esc.gdn_scan(ctx, key, gq, gk, gv, gg, beta, None, gstate, gin.out[0], Tg, Tg, stream=stream), n=5, warm=1)
+    gdn_alg = Tg * workload.H * (ALG_BYTES_PER_TOKEN_HEAD + 4) + 2 * workload.H * 128 * 128 * 4
+    Cc, Wc = 3 * workload.H * 128, 4
+    cx = torch.randn((1, Tg, Cc), device=dev).to(torch.bfloat16)
+    cw = torch.randn((Cc, Wc), device=dev)
+    cst = torch.zeros((1, Cc, Wc - 1), device=dev)
+    cy = torch.empty((1, Tg, Cc), dtype=torch.float32, device=dev)
+    conv_ms, _ = med_ms(lambda: esc.causal_conv(ctx, cx, cw, cst, cst, cy, 1, Tg, Tg, Cc, Wc, esc.CONV_SILU, stream=stream), n=7)
+    conv_alg = Tg * Cc * 6
+    res["gated_delta_rule"] = {"tokens": Tg, "ms": gdn_ms, "tokens_per_s": Tg / (gdn_ms * 1e-3),
+                               "roofline": {"kernel": "esc_gdn_scan_kernel<128> v0 (token-sequential fp32, B1 H16 d128)", "bound": "hbm",
+                                            "achieved": gdn_alg / (gdn_ms * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                                            "frac": gdn_alg / (gdn_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "alg_bytes_per_launch": gdn_alg,
+                                            "note": "bound by the per-token dependency chain (one block reduction + barrier per token), not HBM"},
+                               "causal_conv": {"channels": Cc, "window": Wc, "us": conv_ms * 1e3, "GBps": conv_alg / (conv_ms * 1e-3) / 1e9,
+                                               "frac_of_measured_peak": conv_alg / (conv_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
+                                               "alg_bytes": "2 B read + 4 B written per element"}}
+    del gin, cx, cy
     res["warm_vs_cold"] = {"note": "cold = 18 layers x scan(T=P+64) in one graph; warm = one graph [restore(P) + 18 x scan(64)]; "
                                    "median of 15 (7 at 16k), L2 flushed; the scan only — the paper's TTFT includes the whole model",
                            "by_prefix": table}

@@ -268,6 +268,27 @@ int esc_linattn_scan(esc_ctx* ctx, esc_shape_key key,
                      const float* state_in, float* state_out, void* o,
                      uint64_t T, uint64_t t_stride, uint32_t chunk, void* stream);
 
+/* ---- gated delta rule and convolution state (reading 25) -------------
+ * The recurrence and the convolution window of the paper's own hybrid-model family; both are folds over the whole prefix
+ * and both are capsule rows (the fold state like any esc_linattn_scan state, the convolution window as a fixed-size row).
+ *
+ * esc_gdn_scan: for every (b,h), S_0 = state_in[b,h]:
+ *      u_t = k_t (a_t S_{t-1}) ,  S_t = a_t S_{t-1} + beta_t k_t^T (v_t - u_t) ,  o_t = q_t S_t ,  state_out = S_T
+ * Layouts, alignment and aliasing rules as esc_linattn_scan; `g` holds a_t in (0,1], `beta` [B, T_stride, H] fp32 in [0,1];
+ * keys are expected L2-normalised by the caller.  The key's chunk is ignored: v0 evaluates the plain token-sequential
+ * form in fp32, so restore + continue is bit-identical to the cold run at ANY boundary.  out_dtype must be F32.
+ *
+ * esc_causal_conv: depthwise causal FIR of window W (1..8) over x [B, T_stride, C] bf16 (C % 8 == 0), weights w [C, W] fp32:
+ *      y_t[c] = sum_{i<W} w[c][i] * x_{t-W+1+i}[c]      (+ SiLU with ESC_CONV_SILU),   y [B, T, C] fp32 (dense in T)
+ * where x_s for s < 0 is the carried window state_in [B, C, W-1] fp32 (oldest first; NULL = zeros); state_out receives the
+ * last W-1 inputs after the call and may alias state_in. */
+#define ESC_CONV_SILU 1u
+int esc_gdn_scan(esc_ctx* ctx, esc_shape_key key, const void* q, const void* k, const void* v, const float* g,
+                 const float* beta, const float* state_in, float* state_out, void* o, uint64_t T, uint64_t t_stride,
+                 void* stream);
+int esc_causal_conv(esc_ctx* ctx, const void* x, const float* w, const float* state_in, float* state_out, float* y,
+                    uint32_t B, uint64_t T, uint64_t t_stride, uint32_t C, uint32_t W, uint32_t flags, void* stream);
+
 /* ---- captured replay plan ("replay Graph[key] — never a recapture") -- */
 typedef struct esc_scan_args {
     esc_shape_key key;

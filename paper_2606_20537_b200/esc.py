@@ -28,6 +28,7 @@ TIER_GPU, TIER_HOST = 0, 1
 FORMAT_FP8_E4M3 = 1
 ALL_ROWS = 2**32 - 1
 RESTORE_DEQUANT_EAGER = 1
+CONV_SILU = 1
 
 
 class EscError(RuntimeError):
@@ -86,6 +87,8 @@ _sig = {
     "esc_capsule_valid_end": (C.c_int, [_P, C.c_uint32, C.POINTER(C.c_uint64)]),
     "esc_shape_key_make": (C.c_uint64, [C.c_uint32] * 7),
     "esc_linattn_scan": (C.c_int, [_P, C.c_uint64] + [_P] * 7 + [C.c_uint64, C.c_uint64, C.c_uint32, _P]),
+    "esc_gdn_scan": (C.c_int, [_P, C.c_uint64] + [_P] * 8 + [C.c_uint64, C.c_uint64, _P]),
+    "esc_causal_conv": (C.c_int, [_P] * 6 + [C.c_uint32, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _P]),
     "esc_graph_capture": (C.c_int, [_P, _P, C.c_uint64, C.POINTER(ScanArgs), C.c_uint32, _P, C.POINTER(_P)]),
     "esc_graph_set_capsule": (C.c_int, [_P, _P, _P]),
     "esc_graph_launch": (C.c_int, [_P, _P]),
@@ -308,6 +311,16 @@ def rollback(live, capsule_earlier, stream=None):
 def linattn_scan(ctx, key, q, k, v, g, state_in, state_out, o, T, t_stride, chunk, stream=None):
     _check(lib.esc_linattn_scan(ctx.h, key, _ptr(q), _ptr(k), _ptr(v), _ptr(g), _ptr(state_in), _ptr(state_out),
                                 _ptr(o), T, t_stride, chunk, _stream(stream)), "esc_linattn_scan")
+
+
+def gdn_scan(ctx, key, q, k, v, g, beta, state_in, state_out, o, T, t_stride, stream=None):
+    _check(lib.esc_gdn_scan(ctx.h, key, _ptr(q), _ptr(k), _ptr(v), _ptr(g), _ptr(beta), _ptr(state_in), _ptr(state_out),
+                            _ptr(o), T, t_stride, _stream(stream)), "esc_gdn_scan")
+
+
+def causal_conv(ctx, x, w, state_in, state_out, y, B, T, t_stride, Cch, W, flags=0, stream=None):
+    _check(lib.esc_causal_conv(ctx.h, _ptr(x), _ptr(w), _ptr(state_in), _ptr(state_out), _ptr(y), B, T, t_stride, Cch, W,
+                               flags, _stream(stream)), "esc_causal_conv")
 
 
 def scan_args(key, q, k, v, g, state_in, state_out, o, T, t_stride, chunk):

@@ -81,6 +81,22 @@ def scan_inputs(B, T, H, dk, dv, seed_ids=(0,), gate="fast") -> ScanInputs:
     return ScanInputs(f32_to_bf16_bits(q), f32_to_bf16_bits(k), f32_to_bf16_bits(v), g)
 
 
+def gdn_beta(B, T, H, seed_ids=(0,)) -> np.ndarray:
+    """Write strengths of the gated delta rule (reading 25): beta = sigmoid(x), x ~ N(0,1) per (b,t,h), fp32."""
+    x = rng(*seed_ids, 555).standard_normal((B, T, H))
+    return (1.0 / (1.0 + np.exp(-x))).astype(np.float32)
+
+
+def conv_inputs(B, T, C, W, seed_ids=(0,)):
+    """Short causal convolution inputs: x ~ N(0,1) rounded once to bf16 (bits, uint16 [B,T,C]); taps w ~ N(0,1)/sqrt(W)
+    fp32 [C,W]; a carried window of W-1 earlier bf16-representable inputs as fp32 [B,C,W-1]."""
+    r = rng(*seed_ids, 556)
+    x_bits = f32_to_bf16_bits(r.standard_normal((B, T, C)))
+    w = (r.standard_normal((C, W)) / np.sqrt(W)).astype(np.float32)
+    st = bf16_bits_to_f32(f32_to_bf16_bits(r.standard_normal((B, C, max(W - 1, 0))))).astype(np.float32)
+    return x_bits, w, st
+
+
 def scan_state(B, H, dk, dv, seed_ids=(0,), scale=1.0) -> np.ndarray:
     """A non-zero fp32 start state [B,H,dk,dv] (for S_0 != 0 cases)."""
     return (rng(*seed_ids, 777).standard_normal((B, H, dk, dv)) * scale).astype(np.float32)

@@ -1,0 +1,139 @@
+"""-m gpu parity of esc_gdn_scan (gated delta rule) and esc_causal_conv (convolution state) through the C ABI against
+oracle/gdn_oracle.c (reading 25).  Same bars as the linear-attention scan: o within 2e-3
+(inf-norm ratio), S within 1e-3 (relative Frobenius); restore + continue bit-identical to the cold run — here at ANY
+boundary, the kernel being token-sequential."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_20537_b200 import synth
+from gpu_util import DEV, TOL_O, TOL_S, bits_equal, err_o, err_s, esc_mod, scan_dev_inputs, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def esc():
+    return esc_mod()
+
+
+@pytest.fixture(scope="module")
+def ctx(esc):
+    c = esc.Ctx(0)
+    yield c
+    c.close()
+
+
+def run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv, s0=None, t0=0, n=None):
+    q, k, v, g = dev_in
+    t_stride = q.shape[1]
+    n = T - t0 if n is None else n
+    key = esc.shape_key_make(B, H, dk, dv, esc.DTYPE_BF16, esc.DTYPE_F32, 64)
+    o = torch.full((B, t_stride, H, dv), float("nan"), dtype=torch.float32, device=DEV)
+    s_out = torch.full((B, H, dk, dv), float("nan"), dtype=torch.float32, device=DEV)
+    esc.gdn_scan(ctx, key, q[:, t0:], k[:, t0:], v[:, t0:], g[:, t0:], beta[:, t0:], s0, s_out, o[:, t0:], n, t_stride)
+    torch.cuda.synchronize()
+    return o[:, t0:t0 + n], s_out, o
+
+
+@pytest.mark.parametrize("B,H,dk,dv,T,gate", [
+    (1, 2, 64, 64, 256, "fast"),
+    (2, 3, 128, 128, 300, "fast"),       # ragged: 300 = 4 staged blocks + 44
+    (1, 16, 128, 128, 512, "slow"),      # config-1 head shape, slow decay: the carried state matters throughout
+    (1, 2, 128, 64, 1, "fast"),
+    (1, 1, 64, 128, 65, "one"),
+])
+@pytest.mark.parametrize("with_s0", [False, True])
+def test_gdn_vs_oracle(esc, ctx, B, H, dk, dv, T, gate, with_s0):
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(70, T, H), gate=gate)
+    beta = synth.gdn_beta(B, T, H, seed_ids=(70, T, H))
+    s0 = synth.scan_state(B, H, dk, dv, seed_ids=(71,), scale=0.3) if with_s0 else None
+    o, s, o_full = run_gdn(esc, ctx, scan_dev_inputs(si), to_dev(beta), B, T, H, dk, dv, s0=None if s0 is None else to_dev(s0))
+    q, k, v, g = si.as_f32()
+    o_ref, s_ref = oracle.gdn_recurrence(q, k, v, g, beta, None if s0 is None else s0.astype(np.float64))
+    assert err_o(o.cpu().numpy(), o_ref) <= TOL_O
+    assert err_s(s.cpu().numpy(), s_ref) <= TOL_S
+    assert err_o(o.cpu().numpy(), o_ref) <= 1e-5 and err_s(s.cpu().numpy(), s_ref) <= 1e-5   # fp32 path: far inside the gates
+
+
+def test_gdn_restore_continue_bit_identical_at_any_boundary(esc, ctx):
+    B, H, dk, dv, T = 1, 4, 128, 128, 333
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(72,), gate="slow")
+    beta = to_dev(synth.gdn_beta(B, T, H, seed_ids=(72,)))
+    dev_in = scan_dev_inputs(si)
+    o_cold, s_cold, _ = run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv)
+    for P in (64, 101, 332):            # on and off the staging-block grid
+        _, s_p, _ = run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv, n=P)
+        o_b, s_t, _ = run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv, s0=s_p, t0=P)
+        assert bits_equal(o_b, o_cold[:, P:]) and bits_equal(s_t, s_cold), P
+    # through a capsule: fold state + convolution window as rows of one buffer set
+    key = esc.shape_key_make(B, H, dk, dv, esc.DTYPE_BF16, esc.DTYPE_F32, 64)
+    state = torch.zeros((B, H, dk, dv), dtype=torch.float32, device=DEV)
+    conv_st = torch.randn((B, 256, 3), dtype=torch.float32, device=DEV)
+    live = esc.bufset_create(ctx, [("L00.lin.state", state, state.numel() * 4, state.numel() * 4, 0, 1, 0),
+                                   ("L00.lin.conv", conv_st, conv_st.numel() * 4, conv_st.numel() * 4, 0, 1, 0)])
+    q, k, v, g = dev_in
+    o = torch.zeros((B, T, H, dv), dtype=torch.float32, device=DEV)
+    P = 101
+    esc.gdn_scan(ctx, key, q, k, v, g, beta, None, state, o, P, T)
+    slab = torch.empty(live.capsule_bytes(P)[0], dtype=torch.uint8, device=DEV)
+    cap = esc.snapshot(live, P, 0, slab)
+    keep_conv = conv_st.clone()
+    state.fill_(float("nan"))
+    conv_st.fill_(float("nan"))
+    esc.restore(live, cap)
+    esc.gdn_scan(ctx, key, q[:, P:], k[:, P:], v[:, P:], g[:, P:], beta[:, P:], state, state, o[:, P:], T - P, T)
+    torch.cuda.synchronize()
+    assert bits_equal(o, o_cold) and bits_equal(state, s_cold) and bits_equal(conv_st, keep_conv)
+
+
+def test_gdn_full_size_sampled(esc, ctx):
+    B, H, dk, dv, T = 1, 16, 128, 128, 4096 + 64
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(73,))
+    beta = synth.gdn_beta(B, T, H, seed_ids=(73,))
+    o, s, _ = run_gdn(esc, ctx, scan_dev_inputs(si), to_dev(beta), B, T, H, dk, dv)
+    heads = [0, 9, 15]
+    q, k, v, g = si.as_f32()
+    o_ref, s_ref = oracle.gdn_recurrence(q[:, :, heads], k[:, :, heads], v[:, :, heads], g[:, :, heads], beta[:, :, heads])
+    assert err_o(o[:, :, heads].cpu().numpy(), o_ref) <= TOL_O
+    assert err_s(s[:, heads].cpu().numpy(), s_ref) <= TOL_S
+
+
+def test_gdn_errors(esc, ctx):
+    key_bf = esc.shape_key_make(1, 2, 64, 64, esc.DTYPE_BF16, esc.DTYPE_BF16, 64)
+    x = torch.zeros(16, device=DEV)
+    assert esc.lib.esc_gdn_scan(ctx.h, key_bf, *([x.data_ptr()] * 8), 1, 1, None) == esc.ERR_UNSUPPORTED
+    key = esc.shape_key_make(1, 2, 64, 64, esc.DTYPE_BF16, esc.DTYPE_F32, 64)
+    assert esc.lib.esc_gdn_scan(ctx.h, key, *([x.data_ptr()] * 5), None, None, x.data_ptr(), 1, 1, None) == esc.ERR_INVALID
+    assert esc.lib.esc_gdn_scan(ctx.h, key, *([x.data_ptr() + 2] * 8), 1, 1, None) == esc.ERR_UNALIGNED
+
+
+@pytest.mark.parametrize("B,T,C,W,silu", [(2, 300, 64, 4, False), (1, 1000, 256, 4, True), (1, 2, 8, 4, False), (3, 17, 24, 1, True),
+                                          (1, 64, 6144, 4, True)])
+def test_causal_conv_vs_oracle_and_continuation(esc, ctx, B, T, C, W, silu):
+    x_bits, w, st = synth.conv_inputs(B, T, C, W, seed_ids=(80, T, C))
+    x = to_dev(x_bits.view(np.int16)).view(torch.bfloat16)
+    wd, s_in = to_dev(w), to_dev(st)
+    y = torch.full((B, T, C), float("nan"), dtype=torch.float32, device=DEV)
+    s_out = torch.full((B, C, max(W - 1, 1)), float("nan"), dtype=torch.float32, device=DEV)
+    flags = esc.CONV_SILU if silu else 0
+    esc.causal_conv(ctx, x, wd, s_in if W > 1 else None, s_out, y, B, T, T, C, W, flags)
+    torch.cuda.synchronize()
+    y_ref, s_ref = oracle.causal_conv(synth.bf16_bits_to_f32(x_bits), w, st.astype(np.float64) if W > 1 else None, silu=silu)
+    assert np.abs(y.cpu().numpy() - y_ref).max() <= 1e-5 * max(1.0, np.abs(y_ref).max())
+    if W > 1:
+        assert np.array_equal(s_out.cpu().numpy()[:, :, :W - 1].astype(np.float64), s_ref)    # the window is a copy of inputs: exact
+        # split at P with the carried window, in place (state_in == state_out): bit-identical to the single call
+        for P in (1, T // 2):
+            if P >= T:
+                continue
+            y2 = torch.full_like(y, float("nan"))
+            s_io = s_in.clone()
+            esc.causal_conv(ctx, x, wd, s_io, s_io, y2, B, P, T, C, W, flags)
+            y2b = torch.full((B, T - P, C), float("nan"), dtype=torch.float32, device=DEV)
+            esc.causal_conv(ctx, x[:, P:], wd, s_io, s_io, y2b, B, T - P, T, C, W, flags)
+            torch.cuda.synchronize()
+            # y is dense in T per call: the first call wrote [B, P, C] at the head of y2's storage
+            y_first = y2.view(-1)[: B * P * C].view(B, P, C)
+            assert bits_equal(torch.cat([y_first, y2b], dim=1), y) and bits_equal(s_io[:, :, :W - 1], s_out[:, :, :W - 1])
