@@ -38,8 +38,9 @@ def parse_args():
     ap.add_argument("--impl", default="esc", choices=["esc", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the scan / warm-vs-cold / cpu_baseline extras")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--profile", default=None, choices=["scan", "restore"],
-                    help="ncu driver: launch only the cold 16448-token scan (x3) or only the 66 MiB restore (x5); no JSON line")
+    ap.add_argument("--profile", default=None, choices=["scan", "restore", "suffix"],
+                    help="ncu driver: launch only the cold 16448-token scan (x3), only the 66 MiB restore (x5) or only the 18 "
+                         "64-token suffix scans (x2); no JSON line")
     return ap.parse_args()
 
 
@@ -321,7 +322,9 @@ def run_esc(args):
     sfx_gbs = sfx_alg / (sfx_us * 1e-6) / 1e9
     roof_sfx = {"kernel": "esc_scan_tc_kernel<128,64,4,float> (B1 H16 d128, T=64 suffix: one chunk per (b,h); 18 launches per step)",
                 "bound": "hbm", "achieved": sfx_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": sfx_gbs / pk["hbm_gbs"],
-                "peak_source": pk["source"], "traffic": None, "us_per_launch": sfx_us, "alg_bytes_per_launch": sfx_alg,
+                "peak_source": pk["source"], "traffic": 1.89e6, "us_per_launch": sfx_us, "alg_bytes_per_launch": sfx_alg,
+                "traffic_note": "ncu r01h (profiles/r01h_suffix_scan_ncu_full.txt): dram read 1.89 MB, write 0 in the kernel's window "
+                                "(state and outputs still dirty in L2 at kernel end)",
                 "share_of_step": ms_suffix / ms_step,
                 "note": "latency-bound by construction: 3.4 MB per launch is 0.5 us of HBM time; the launch is one chunk of "
                         "the dependent pipeline (TMA -> P -> scores -> O2 -> store) plus setup/teardown"}
@@ -412,7 +415,7 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
                            "tokens_per_s_18_layer_cold_graph": T / (cold_ms * 1e-3), "alg_TFLOPs": flops / (one_ms * 1e-3) / 1e12}
             res["roofline_scan_cold"] = {"kernel": "esc_scan_tc_kernel<128,64,4,float> (B1 H16 d128 T=16448 chunk 64: BASELINE config 2 cold scan, one layer)", "bound": "hbm",
                                     "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": gbs / pk["hbm_gbs"],
-                                    "peak_source": pk["source"], "traffic": None, "us_per_launch": one_ms * 1e3,
+                                    "peak_source": pk["source"], "traffic": 308.4e6, "us_per_launch": one_ms * 1e3,
                                     "alg_bytes_per_launch": alg}
         cold_graph.destroy()
         warm_graph.destroy()
@@ -524,6 +527,15 @@ def run_profile(args):
         key = esc.shape_key_make(1, 16, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
         for _ in range(3):
             esc.linattn_scan(ctx, key, *full.dev[0], None, sess.states[0], full.out[0], T, T, CHUNK, stream=stream)
+    elif args.profile == "suffix":
+        sess = workload.HybridSession(ctx, P_STEP + SUFFIX, seed=0)
+        inputs = workload.SuffixInputs(N_LINEAR, SUFFIX, seed=0)
+        layers, key = workload.scan_layers(sess, inputs, CHUNK)
+        for _ in range(2):
+            for n in range(N_LINEAR):
+                q, k, v, g = inputs.dev[n]
+                esc.linattn_scan(ctx, key, q, k, v, g, sess.states[n], sess.states[n], inputs.out[n], SUFFIX, SUFFIX, CHUNK,
+                                 stream=stream)
     else:
         sess = workload.HybridSession(ctx, P_STEP + SUFFIX, seed=0)
         slabs = [sess.new_slab(P_STEP) for _ in range(5)]
