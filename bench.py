@@ -508,6 +508,27 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
                                                "frac_of_measured_peak": conv_alg / (conv_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
                                                "alg_bytes": "2 B read + 4 B written per element"}}
     del gin, cx, cy
+    # ---- BASELINE config 4: scan sweep (B 1-4, H16, d128, T 2k-64k, chunk 64/128), device-generated inputs of the same
+    # distributions (timing only; parity at these shapes is tests/test_gpu_scan.py::test_config4_sweep_points_sampled) ----
+    sweep = []
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(20537)
+    for (Bs, Ts, Cs) in ((1, 2048, 64), (1, 8192, 64), (1, 32768, 64), (1, 65536, 64), (4, 8192, 64), (4, 32768, 64), (1, 8192, 128),
+                         (1, 65536, 128), (4, 32768, 128)):
+        sq = torch.nn.functional.normalize(torch.randn((Bs, Ts, workload.H, 128), device=dev, generator=gen), dim=-1).to(torch.bfloat16)
+        sk = torch.nn.functional.normalize(torch.randn((Bs, Ts, workload.H, 128), device=dev, generator=gen), dim=-1).to(torch.bfloat16)
+        sv = torch.randn((Bs, Ts, workload.H, 128), device=dev, generator=gen).to(torch.bfloat16)
+        sg = torch.sigmoid(-torch.randn((Bs, Ts, workload.H), device=dev, generator=gen)).clamp_min(1e-30)
+        so = torch.empty((Bs, Ts, workload.H, 128), dtype=torch.float32, device=dev)
+        ss = torch.empty((Bs, workload.H, 128, 128), dtype=torch.float32, device=dev)
+        skey = esc.shape_key_make(Bs, workload.H, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, Cs)
+        ms_, _ = med_ms(lambda: esc.linattn_scan(ctx, skey, sq, sk, sv, sg, None, ss, so, Ts, Ts, Cs, stream=stream), n=5, warm=1)
+        alg_ = Bs * Ts * workload.H * ALG_BYTES_PER_TOKEN_HEAD + 2 * Bs * workload.H * 128 * 128 * 4
+        sweep.append({"B": Bs, "T": Ts, "chunk": Cs, "ms": ms_, "tokens_per_s": Bs * Ts / (ms_ * 1e-3),
+                      "frac_of_hbm_roofline": alg_ / (ms_ * 1e-3) / 1e9 / pk["hbm_gbs"]})
+        del sq, sk, sv, sg, so, ss
+        torch.cuda.empty_cache()
+    res["scan_sweep"] = sweep
     res["warm_vs_cold"] = {"note": "cold = 18 layers x scan(T=P+64) in one graph; warm = one graph [restore(P) + 18 x scan(64)]; "
                                    "median of 15 (7 at 16k), L2 flushed; the scan only — the paper's TTFT includes the whole model",
                            "by_prefix": table}

@@ -261,7 +261,8 @@ esc_shape_key esc_shape_key_make(uint32_t B, uint32_t H, uint32_t d_k, uint32_t 
  * chunk is short).  T == 0 copies state_in to state_out.  state_in may be NULL (= zeros)
  * and may alias state_out.  q, k, v, o and the states 16-byte aligned, g 4-byte aligned
  * (ESC_ERR_UNALIGNED).
- * `chunk` must equal the key's chunk (ESC_ERR_MISMATCH).  One kernel launch on `stream`.
+ * `chunk` must equal the key's chunk (ESC_ERR_MISMATCH): it is the alignment grid of restore boundaries the caller
+ * commits to; the kernel's internal token tile is 64 for both values.  One kernel launch on `stream`.
  */
 int esc_linattn_scan(esc_ctx* ctx, esc_shape_key key,
                      const void* q, const void* k, const void* v, const float* g,
