@@ -23,12 +23,12 @@
 // Ring and A-buffer reuse are therefore cluster-wide events: stage / A-buffer "empty" barriers count
 // tcgen05.commit arrivals multicast from all CS CTAs.  The score path (P -> A -> O2) has its own buffers
 // (NB of each, O2 reads V from a copy the V~ warps make), so it never holds an input stage.
-// What bounds it (r01, ncu + clock64 traces): shared-memory bandwidth.  Per chunk a CTA moves ~160 KB
-// through its shared memory (34 KB TMA writes, 84 KB tcgen05.mma operand reads — Q twice, K, A, each for
-// a 16..32-column B operand — 24 KB of A-slice exchange, 16 KB of V~ / S operand writes) = ~1270 cycles at
-// 128 B/clk against a measured period of ~1400; ALU, MUFU, issue-slot and spin-wait ablations moved
-// nothing.  The d_v split that fills the SMs at B H = 16 is what makes the A operands (Q, K, A) be
-// re-read per 16 output columns.
+// What bounds it (r01: ncu, clock64 traces, per-warp busy/wait accounting, ablation builds): the four MMA-issuing
+// threads.  They are the busiest threads of the CTA (1200-1400 of a 1400-cycle period per chunk; every other role
+// 600-1000): 28 small tcgen05.mma (M = 64, N = 16..32) and 11 tcgen05.commit per chunk at ~110 / ~130 cycles of issuing-
+// thread time each, where the tensor pipe itself needs 13-23 cycles per such MMA (microbenchmark).  DRAM, tensor pipe,
+// issue slots, L2, DSMEM and the TMA loads each have slack (removing any one of them changes nothing).  The d_v split
+// that fills the SMs at B H = 16 is what makes the MMAs this small; DESIGN.md 6.2 lists what was tried.
 //
 // Warp roles (22 warps, mbarrier-synchronised software pipeline, no CTA-wide barrier in the loop):
 //   warp 0         TMA producer (multicast Q/K row slices, own V slice; L2 prefetch ahead)
