@@ -189,72 +189,72 @@ __global__ void __launch_bounds__(kGdnThreads) esc_gdn_scan_kernel(const __nv_bf
 }
 
 // ---- short causal depthwise convolution, window W <= 8 -----------------------------------------------------
-// Bound: HBM (2 B read + 4 B written per element).  A thread owns 8 consecutive channels (one 16-byte bf16 vector; a
-// warp reads 512 contiguous bytes of a token row) and walks kConvRun consecutive tokens with the W-1 previous input
+// Bound: HBM (2 B read + 4 B written per element).  A thread owns 4 consecutive channels (one 8-byte bf16 vector; a
+// warp reads 256 contiguous bytes of a token row) and walks kConvRun consecutive tokens with the W-1 previous input
 // vectors and its 8 x W taps in registers, so every input vector is loaded once per run (+ W-1 to prime the window).
 constexpr int kConvMaxW = 8;
 constexpr int kConvRun = 64;      // tokens per thread
 constexpr int kConvThreads = 128;
+constexpr int kConvCPT = 4;       // channels per thread (8-byte bf16 vectors: a warp reads 256 contiguous bytes of a token row)
 
-__device__ __forceinline__ void bf16x8_to_f32(const uint4& raw, float (&x)[8]) {
-    const uint32_t r[4] = {raw.x, raw.y, raw.z, raw.w};
-#pragma unroll
-    for (int j = 0; j < 8; ++j) x[j] = __uint_as_float((j & 1) ? (r[j >> 1] & 0xFFFF0000u) : (r[j >> 1] << 16));
+__device__ __forceinline__ void bf16x4_to_f32(const uint2& raw, float (&x)[4]) {
+    x[0] = __uint_as_float(raw.x << 16); x[1] = __uint_as_float(raw.x & 0xFFFF0000u);
+    x[2] = __uint_as_float(raw.y << 16); x[3] = __uint_as_float(raw.y & 0xFFFF0000u);
 }
 
 template <int W>
 __global__ void __launch_bounds__(kConvThreads) esc_causal_conv_kernel(const __nv_bfloat16* __restrict__ x, const float* __restrict__ w,
                                                                        const float* __restrict__ state_in, float* __restrict__ y,
                                                                        uint64_t T, uint64_t t_stride, uint32_t C, uint32_t silu) {
-    const uint32_t c8 = blockIdx.x * kConvThreads + threadIdx.x;
-    if (c8 >= C / 8) return;
+    constexpr int P = kConvCPT;
+    const uint32_t cg = blockIdx.x * kConvThreads + threadIdx.x;   // channel group
+    if (cg >= C / P) return;
     const uint32_t b = blockIdx.z;
     const uint64_t t_begin = (uint64_t)blockIdx.y * kConvRun;
     const uint64_t t_end = t_begin + kConvRun < T ? t_begin + kConvRun : T;
-    float wt[W][8];   // wt[i][j] = tap i of channel 8 c8 + j
+    float wt[W][P];   // wt[i][j] = tap i of channel P cg + j
 #pragma unroll
-    for (int j = 0; j < 8; ++j)
+    for (int j = 0; j < P; ++j)
 #pragma unroll
-        for (int i = 0; i < W; ++i) wt[i][j] = w[(size_t)(c8 * 8 + j) * W + i];
+        for (int i = 0; i < W; ++i) wt[i][j] = w[(size_t)(cg * P + j) * W + i];
     // win[i] = input at position t - (W-1) + i for the current t; primed with the W-1 inputs before t_begin
-    float win[W][8];
+    float win[W][P];
 #pragma unroll
     for (int i = 0; i < W - 1; ++i) {
         const int64_t s = (int64_t)t_begin - (W - 1) + i;
         if (s >= 0) {
-            bf16x8_to_f32(*reinterpret_cast<const uint4*>(x + ((size_t)b * t_stride + (uint64_t)s) * C + c8 * 8), win[i]);
+            bf16x4_to_f32(*reinterpret_cast<const uint2*>(x + ((size_t)b * t_stride + (uint64_t)s) * C + cg * P), win[i]);
         } else {
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
-                win[i][j] = state_in ? state_in[((size_t)b * C + c8 * 8 + j) * (W - 1) + (uint32_t)((int64_t)(W - 1) + s)] : 0.f;
+            for (int j = 0; j < P; ++j)
+                win[i][j] = state_in ? state_in[((size_t)b * C + cg * P + j) * (W - 1) + (uint32_t)((int64_t)(W - 1) + s)] : 0.f;
         }
     }
-    const __nv_bfloat16* xp = x + ((size_t)b * t_stride + t_begin) * C + c8 * 8;
-    float* yp = y + ((size_t)b * T + t_begin) * C + c8 * 8;
+    const __nv_bfloat16* xp = x + ((size_t)b * t_stride + t_begin) * C + cg * P;
+    float* yp = y + ((size_t)b * T + t_begin) * C + cg * P;
     constexpr int U = 4;   // loads in flight per thread
     for (uint64_t t = t_begin; t < t_end; t += U) {
-        uint4 raw[U];
+        uint2 raw[U];
 #pragma unroll
         for (int u = 0; u < U; ++u)
-            if (t + u < t_end) raw[u] = *reinterpret_cast<const uint4*>(xp + (size_t)u * C);
+            if (t + u < t_end) raw[u] = *reinterpret_cast<const uint2*>(xp + (size_t)u * C);
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             if (t + u < t_end) {
-                bf16x8_to_f32(raw[u], win[W - 1]);
-                float acc[8];
+                bf16x4_to_f32(raw[u], win[W - 1]);
+                float acc[P];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < P; ++j) {
                     float s_ = 0.f;
 #pragma unroll
                     for (int i = 0; i < W; ++i) s_ = fmaf(wt[i][j], win[i][j], s_);
                     acc[j] = silu ? s_ / (1.f + expf(-s_)) : s_;
                 }
-                reinterpret_cast<float4*>(yp + (size_t)u * C)[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-                reinterpret_cast<float4*>(yp + (size_t)u * C)[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+                *reinterpret_cast<float4*>(yp + (size_t)u * C) = make_float4(acc[0], acc[1], acc[2], acc[3]);
 #pragma unroll
                 for (int i = 0; i < W - 1; ++i)
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) win[i][j] = win[i + 1][j];
+                    for (int j = 0; j < P; ++j) win[i][j] = win[i + 1][j];
             }
         }
         xp += (size_t)U * C;
@@ -335,7 +335,7 @@ int esc_causal_conv(esc_ctx* ctx, const void* x, const float* w, const float* st
     if ((((uintptr_t)x | (uintptr_t)y) & 15u) || (((uintptr_t)w | (uintptr_t)state_in | (uintptr_t)state_out) & 3u)) return ESC_ERR_UNALIGNED;
     if (T > 0) {
         if (B > 65535) return ESC_ERR_UNSUPPORTED;
-        dim3 grid((C / 8 + kConvThreads - 1) / kConvThreads, (uint32_t)((T + kConvRun - 1) / kConvRun), B);
+        dim3 grid((C / kConvCPT + kConvThreads - 1) / kConvThreads, (uint32_t)((T + kConvRun - 1) / kConvRun), B);
         conv_kernel_for(W)<<<grid, kConvThreads, 0, (cudaStream_t)stream>>>((const __nv_bfloat16*)x, w, state_in, y, T, t_stride, C,
                                                                             flags & ESC_CONV_SILU);
         ESC_CUDA(cudaGetLastError());
