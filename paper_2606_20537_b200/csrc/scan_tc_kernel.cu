@@ -361,17 +361,21 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
         // ================= issuer: P[:, key0 .. key0+NA) = Q K[key0 .. key0+NA)^T =================
         if (lane == 0) {
             constexpr uint32_t idP = idesc_bf16(C, NA, 0, 0);
+            // descriptors of stage 0; per chunk / per MMA they are only advanced (the issuing thread's instruction count per
+            // MMA is what paces the kernel)
+            const uint64_t dQ0 = smem_desc(sm_a + L::stage_off, 16, 1024, kSwz128);
+            const uint64_t dK0 = smem_desc(sm_a + L::stage_off + L::q_bytes + key0 * 128, 16, 1024, kSwz128);
             for (uint32_t c = 0; c < n_chunks; ++c) {
                 const uint32_t s = c % NS, pb = c % NB;
                 mbar_wait(&bars[BI.full + s], (c / NS) & 1);
                 mbar_wait(&bars[BI.p_empty + pb], ((c / NB) & 1) ^ 1);
                 tc_fence_after_sync();
-                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes, ka = qa + L::q_bytes + key0 * 128;
+                const uint64_t dQ = smem_desc_advance(dQ0, s * L::stage_bytes), dK = smem_desc_advance(dK0, s * L::stage_bytes);
+                const uint32_t dP = tb + L::tm_p + pb * 32;
 #pragma unroll
                 for (int ks = 0; ks < DK / 16; ++ks) {
                     const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
-                    mma_bf16_ss(tb + L::tm_p + pb * 32, smem_desc(qa + off, 16, 1024, kSwz128),
-                                smem_desc(ka + off, 16, 1024, kSwz128), idP, ks > 0);
+                    mma_bf16_ss(dP, smem_desc_advance(dQ, off), smem_desc_advance(dK, off), idP, ks > 0);
                 }
                 mma_commit(&bars[BI.p_full + pb]);
                 mma_commit_mc(&bars[BI.empty + s], kAll);
@@ -382,6 +386,8 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
         // ================= issuer: O1 = Q [S_hi | S_lo] — the only MMA that reads the carried state =================
         if (lane == 0) {
             constexpr uint32_t idO1 = idesc_bf16(C, kTcNM, 0, 1);
+            const uint64_t dQ0 = smem_desc(sm_a + L::stage_off, 16, 1024, kSwz128);
+            const uint64_t dS0 = smem_desc(sm_a + L::s_off, 128, SBO_S, kSwzNone);
             for (uint32_t c = 0; c < n_chunks; ++c) {
                 const uint32_t s = c % NS, ob = c & 1, sb = c % NSB;
                 mbar_wait(&bars[BI.full + s], (c / NS) & 1);
@@ -389,12 +395,12 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 mbar_wait(&bars[BI.s_full + sb], (c / NSB) & 1);
                 tc_fence_after_sync();
                 TC_TRACE(2, c);
-                const uint32_t qa = sm_a + L::stage_off + s * L::stage_bytes, sa = sm_a + L::s_off + sb * L::s_bytes;
+                const uint64_t dQ = smem_desc_advance(dQ0, s * L::stage_bytes), dS = smem_desc_advance(dS0, sb * L::s_bytes);
+                const uint32_t dO = tb + L::tm_o1 + ob * 32;
 #pragma unroll
                 for (int ks = 0; ks < DK / 16; ++ks) {
                     const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
-                    mma_bf16_ss(tb + L::tm_o1 + ob * 32, smem_desc(qa + off, 16, 1024, kSwz128),
-                                smem_desc(sa + 2 * ks * 128, 128, SBO_S, kSwzNone), idO1, ks > 0);
+                    mma_bf16_ss(dO, smem_desc_advance(dQ, off), smem_desc_advance(dS, 2 * ks * 128), idO1, ks > 0);
                 }
                 mma_commit(&bars[BI.s_empty + sb]);
                 mma_commit(&bars[BI.o1_full + ob]);
@@ -405,6 +411,8 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
         // ================= issuer: U = K^T [V~_hi | V~_lo] (A operand = the K tile read MN-major) =================
         if (lane == 0) {
             constexpr uint32_t idU = idesc_bf16(DK, kTcNM, 1, 1);
+            const uint64_t dK0 = smem_desc(sm_a + L::stage_off + L::q_bytes, L::half_bytes, 1024, kSwz128);
+            const uint64_t dV0 = smem_desc(sm_a + L::vt_off, 128, SBO_V, kSwzNone);
             for (uint32_t c = 0; c < n_chunks; ++c) {
                 const uint32_t s = c % NS, pb = c % NB, ob = c & 1;
                 mbar_wait(&bars[BI.full + s], (c / NS) & 1);
@@ -412,11 +420,11 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 mbar_wait(&bars[BI.vt_full + pb], (c / NB) & 1);   // the V~ warps are then also done with the stage's V tile
                 tc_fence_after_sync();
                 TC_TRACE(3, c);
-                const uint32_t ka = sm_a + L::stage_off + s * L::stage_bytes + L::q_bytes, vt = sm_a + L::vt_off + pb * L::vt_bytes;
+                const uint64_t dK = smem_desc_advance(dK0, s * L::stage_bytes), dV = smem_desc_advance(dV0, pb * L::vt_bytes);
+                const uint32_t dU = tb + L::tm_u + ob * 32;
 #pragma unroll
                 for (int ks = 0; ks < C / 16; ++ks)
-                    mma_bf16_ss(tb + L::tm_u + ob * 32, smem_desc(ka + 2 * ks * 1024, L::half_bytes, 1024, kSwz128),
-                                smem_desc(vt + 2 * ks * 128, 128, SBO_V, kSwzNone), idU, ks > 0);
+                    mma_bf16_ss(dU, smem_desc_advance(dK, 2 * ks * 1024), smem_desc_advance(dV, 2 * ks * 128), idU, ks > 0);
                 mma_commit(&bars[BI.u_full + ob]);
                 mma_commit(&bars[BI.vt_empty + pb]);
                 mma_commit_mc(&bars[BI.empty + s], kAll);
@@ -426,6 +434,8 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
         // ================= issuer: O2 = A_hi V + A_lo V (B operand = the V tile copy, MN-major, 32B swizzle) =================
         if (lane == 0) {
             constexpr uint32_t idO2 = idesc_bf16(C, kTcDVT, 0, 1);
+            const uint64_t dA0 = smem_desc(sm_a + L::a_off, L::a_lbo, 128, kSwzNone);
+            const uint64_t dV0 = smem_desc(sm_a + L::vt_off + L::vc_off, 512, 256, kSwz32);
             for (uint32_t c = 0; c < n_chunks; ++c) {
                 const uint32_t pb = c % NB, ob = c & 1;
                 mbar_wait(&bars[BI.o_empty + ob], ((c >> 1) & 1) ^ 1);
@@ -433,13 +443,14 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 mbar_wait(&bars[BI.a_full + pb], (c / NB) & 1);    // own slice written + every peer's slice landed
                 tc_fence_after_sync();
                 TC_TRACE(4, c);
-                const uint32_t va = sm_a + L::vt_off + pb * L::vt_bytes + L::vc_off, aa = sm_a + L::a_off + pb * L::a_bytes;
+                const uint64_t dA = smem_desc_advance(dA0, pb * L::a_bytes), dV = smem_desc_advance(dV0, pb * L::vt_bytes);
+                const uint32_t dO = tb + L::tm_o2 + ob * 16;
 #pragma unroll
                 for (int term = 0; term < 2; ++term) {
 #pragma unroll
                     for (int ks = 0; ks < C / 16; ++ks)
-                        mma_bf16_ss(tb + L::tm_o2 + ob * 16, smem_desc(aa + term * L::a_term + 2 * ks * L::a_lbo, L::a_lbo, 128, kSwzNone),
-                                    smem_desc(va + 2 * ks * 256, 512, 256, kSwz32), idO2, (term | ks) > 0);
+                        mma_bf16_ss(dO, smem_desc_advance(dA, term * L::a_term + 2 * ks * L::a_lbo), smem_desc_advance(dV, 2 * ks * 256), idO2,
+                                    (term | ks) > 0);
                 }
                 mma_commit(&bars[BI.o2_full + ob]);
                 mma_commit(&bars[BI.vt_empty + pb]);

@@ -212,6 +212,9 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes
     d |= (uint64_t)swizzle << 61;
     return d;
 }
+// the same descriptor `bytes` further on (the start-address field holds addr >> 4 in its low 14 bits; shared memory is < 256 KB,
+// so the sum never carries out of the field): one add per MMA instead of rebuilding the descriptor
+__device__ __forceinline__ uint64_t smem_desc_advance(uint64_t desc, uint32_t bytes) { return desc + (uint64_t)(bytes >> 4); }
 // instruction descriptor, kind::f16: D fp32 (bits 4-5 = 1), A/B bf16 (bits 7-9 / 10-12 = 1), majors (0 = K, 1 = MN),
 // N >> 3 at bit 17, M >> 4 at bit 24
 __host__ __device__ constexpr uint32_t idesc_bf16(uint32_t M, uint32_t N, uint32_t a_mn_major, uint32_t b_mn_major) {
