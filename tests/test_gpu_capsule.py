@@ -287,3 +287,40 @@ def test_host_tier_capsule_in_graph(esc, ctx):
         oracle.capsule_restore(live.oracle_rows(), P, ref)
         live.assert_equals_host()
     graph.destroy()
+
+
+def test_seeded_layout_fuzz_bit_exact(esc, ctx):
+    # 12 seeded random buffer sets (odd sizes, mixed fixed / per-token rows, multi-segment rows, unaligned base offsets):
+    # snapshot -> dirty -> restore and a 3-way fork, byte-exact against the memcpy oracle
+    rng = np.random.default_rng(20538)
+    for it in range(12):
+        specs = []
+        t_max = int(rng.integers(8, 200))
+        for r in range(int(rng.integers(1, 9))):
+            kind = int(rng.integers(0, 3))
+            if kind == 0:
+                nb = int(rng.integers(1, 5000))
+                specs.append(synth.RowSpec("r%02d.fixed" % r, nb, nb, 0, 1, 0))
+            elif kind == 1:
+                bpt = int(rng.integers(1, 300))
+                specs.append(synth.RowSpec("r%02d.tok" % r, t_max * bpt, 0, bpt, 1, 0))
+            else:
+                bpt, nseg = int(rng.integers(1, 120)), int(rng.integers(2, 5))
+                stride = t_max * bpt + int(rng.integers(0, 40))
+                specs.append(synth.RowSpec("r%02d.seg" % r, stride * nseg, 0, bpt, nseg, stride))
+        P = int(rng.integers(0, t_max + 1))
+        live = LiveSet(esc, ctx, specs, (30, it), offset_bytes=int(rng.choice([0, 0, 1, 3, 16])))
+        slab = _slab(live.set.capsule_bytes(P)[0] + 256)
+        cap = esc.snapshot(live.set, P, 0, slab)
+        torch.cuda.synchronize()
+        ref = _check_snapshot_matches_oracle(live, slab, P)
+        live.fill(31, it, pattern=0xFF)
+        esc.restore(live.set, cap)
+        oracle.capsule_restore(live.oracle_rows(), P, ref)
+        live.assert_equals_host()
+        forks = [LiveSet(esc, ctx, specs, (32, it, f), offset_bytes=int(rng.choice([0, 2]))) for f in range(3)]
+        esc.fork(cap, [f.set for f in forks])
+        for f in forks:
+            oracle.capsule_restore(f.oracle_rows(), P, ref)
+            f.assert_equals_host()
+        cap.destroy()
