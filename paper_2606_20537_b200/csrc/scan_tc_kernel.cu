@@ -76,7 +76,7 @@ __device__ __forceinline__ long long tc_gtime() { long long t; asm volatile("mov
 #define TC_TRACE_L(ev, id) do { } while (0)
 #endif
 
-template <int DK, int C>
+template <int DK, int C, int CS>
 struct TcCfg {
     static constexpr int NS = (C == 64) ? 4 : 2;          // input stages
     static constexpr int NB = (C == 64) ? 3 : 1;          // P / A / V~ (+ V copy) buffers
@@ -105,12 +105,13 @@ struct TcCfg {
     static constexpr uint32_t bar_off = gate_off + 2 * 2 * kGateBatch * 4;
     static constexpr uint32_t n_bars = 2 * NS + 6 * NB + 2 * NSB + 14;
     static constexpr uint32_t total = bar_off + 64 * 8 + 16 + 1024;             // + alignment slack
-    static constexpr uint32_t tmem_cols = 256;
-    static constexpr uint32_t tm_p = 0;                    // [NB] x 32 columns (a slice has C/CS <= 32)
-    static constexpr uint32_t tm_u = 96;                   // [2] x 32
-    static constexpr uint32_t tm_o1 = 160;                 // [2] x 32
-    static constexpr uint32_t tm_o2 = 224;                 // [2] x 16
-    static_assert(NB * 32 <= tm_u, "TMEM budget");
+    static constexpr uint32_t p_cols = (C / CS <= 32) ? 32 : 64;   // TMEM columns of one P buffer (a slice has C/CS keys)
+    static constexpr uint32_t tm_p = 0;                    // [NB] x p_cols
+    static constexpr uint32_t tm_u = NB * p_cols;          // [2] x 32
+    static constexpr uint32_t tm_o1 = tm_u + 64;           // [2] x 32
+    static constexpr uint32_t tm_o2 = tm_o1 + 64;          // [2] x 16
+    static constexpr uint32_t tmem_cols = (tm_o2 + 32 <= 256) ? 256 : 512;
+    static_assert(tm_o2 + 32 <= tmem_cols, "TMEM budget");
     static_assert(stage_bytes % 1024 == 0, "stages must keep 1024-byte alignment (128B swizzle)");
     static_assert(n_bars <= 64, "barrier area");
     static_assert(total <= 232448, "shared memory budget");
@@ -120,9 +121,9 @@ struct TcBars {   // indices into the mbarrier array
     int full, empty, p_full, p_empty, a_full, a_empty, vt_full, vt_empty, s_full, s_empty, o1_full, o2_full, o_empty, u_full,
         u_empty, g_full, g_empty;
 };
-template <int DK, int C>
+template <int DK, int C, int CS>
 __device__ __forceinline__ constexpr TcBars tc_bars() {
-    using L = TcCfg<DK, C>;
+    using L = TcCfg<DK, C, CS>;
     TcBars b{};
     int i = 0;
     b.full = i; i += L::NS;
@@ -177,7 +178,8 @@ template <int NA>
 __device__ __forceinline__ void tmem_ld_slice(uint32_t addr, uint32_t* r) {
     if constexpr (NA == 8) tmem_ld_16x256b_x1(addr, r);
     else if constexpr (NA == 16) tmem_ld_16x256b_x2(addr, r);
-    else tmem_ld_16x256b_x4(addr, r);
+    else if constexpr (NA == 32) tmem_ld_16x256b_x4(addr, r);
+    else tmem_ld_16x256b_x8(addr, r);
 }
 
 template <int DK, int C, int CS, typename OutT>
@@ -185,13 +187,13 @@ __global__ void __launch_bounds__(kTcThreads, 1)
 esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tk,
                    const __grid_constant__ CUtensorMap tv, const float* __restrict__ g, const float* state_in,
                    float* state_out, OutT* __restrict__ o, uint32_t H, uint32_t DV, uint64_t T, uint64_t t_stride) {
-    using L = TcCfg<DK, C>;
-    constexpr TcBars BI = tc_bars<DK, C>();
+    using L = TcCfg<DK, C, CS>;
+    constexpr TcBars BI = tc_bars<DK, C, CS>();
     constexpr int NS = L::NS, NB = L::NB, NSB = L::NSB, CPB = L::CPB;
     constexpr int NA = C / CS;                      // keys per score slice = Q / K rows this CTA loads
     constexpr uint16_t kAll = (uint16_t)((1u << CS) - 1);
     constexpr uint32_t SBO_V = (C / 8) * 128, SBO_S = (DK / 8) * 128;
-    static_assert(NA == 8 || NA == 16 || NA == 32, "slice width");
+    static_assert(NA == 8 || NA == 16 || NA == 32 || NA == 64, "slice width");
     static_assert(C == 128 ? NA >= 16 : true, "an M = 128 MMA needs N % 16 == 0");
 
     extern __shared__ uint8_t smem_raw[];
@@ -202,7 +204,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     float* gate = reinterpret_cast<float*>(sm + L::gate_off);   // [2][2][256]: b2 then eb per slot
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t rank = cluster_ctarank();   // clusters are CS consecutive d_v slices (blockIdx.x) of one (b, h)
+    const uint32_t rank = CS > 1 ? cluster_ctarank() : 0u;   // clusters are CS consecutive d_v slices (blockIdx.x) of one (b, h)
     const uint32_t bh = blockIdx.y, b = bh / H, h = bh % H, dv0 = blockIdx.x * kTcDVT;
     const uint32_t key0 = rank * NA;    // first key (= first Q / K row) of this CTA's slice
     const uint32_t n_chunks = (uint32_t)((T + C - 1) / C);
@@ -218,6 +220,11 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     // griddepcontrol.wait below, i.e. after the preceding kernel has completed and flushed.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
+    // commit that every CTA of the cluster must see (stage / A-buffer reuse)
+    auto commit_all = [&](uint64_t* bar) {
+        if constexpr (CS > 1) mma_commit_mc(bar, kAll);
+        else mma_commit(bar);
+    };
     // TMA producer steps (warp 0, lane 0)
     auto tma_prefetch_chunk = [&](uint32_t c) {   // pull this CTA's share of chunk c into L2
         const int t0 = (int)(c * C);
@@ -236,9 +243,14 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
         const int t0 = (int)(c * C);
 #pragma unroll
         for (int hh = 0; hh < L::NH; ++hh) {
-            tma_load_4d_mc(st + hh * L::half_bytes + key0 * 128, &tq, full, hh * 64, (int)h, t0 + (int)key0, (int)b, kAll);
-            tma_load_4d_mc(st + L::q_bytes + hh * L::half_bytes + key0 * 128, &tk, full, hh * 64, (int)h, t0 + (int)key0, (int)b,
-                           kAll);
+            if constexpr (CS > 1) {
+                tma_load_4d_mc(st + hh * L::half_bytes + key0 * 128, &tq, full, hh * 64, (int)h, t0 + (int)key0, (int)b, kAll);
+                tma_load_4d_mc(st + L::q_bytes + hh * L::half_bytes + key0 * 128, &tk, full, hh * 64, (int)h, t0 + (int)key0, (int)b,
+                               kAll);
+            } else {
+                tma_load_4d(st + hh * L::half_bytes, &tq, full, hh * 64, (int)h, t0, (int)b);
+                tma_load_4d(st + L::q_bytes + hh * L::half_bytes, &tk, full, hh * 64, (int)h, t0, (int)b);
+            }
         }
         tma_load_4d(st + 2 * L::q_bytes, &tv, full, (int)dv0, (int)h, t0, (int)b);
         TC_TRACE(0, c);
@@ -263,12 +275,16 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     }
     if (warp == 2) tmem_alloc(tmem_slot, L::tmem_cols);
     // A buffers: blocks above the causal diagonal are never written by any CTA and must read as zero
-    for (uint32_t i = threadIdx.x; i < NB * L::a_bytes / 16; i += kTcThreads)
-        reinterpret_cast<uint4*>(sm + L::a_off)[i] = make_uint4(0, 0, 0, 0);
+    // (a CTA on its own, CS = 1, writes every element of A itself, the masked ones as zeros)
+    if constexpr (CS > 1) {
+        for (uint32_t i = threadIdx.x; i < NB * L::a_bytes / 16; i += kTcThreads)
+            reinterpret_cast<uint4*>(sm + L::a_off)[i] = make_uint4(0, 0, 0, 0);
+    }
     fence_proxy_async_smem();
     tc_fence_before_sync();
     // every CTA's barriers are initialised and its A buffers zeroed before any peer multicasts / copies into them
-    cluster_sync();
+    if constexpr (CS > 1) cluster_sync();
+    else __syncthreads();
     tc_fence_after_sync();
     const uint32_t tb = *tmem_slot;
     asm volatile("griddepcontrol.wait;" ::: "memory");   // ---- global memory may be touched from here on ----
@@ -371,14 +387,14 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 mbar_wait(&bars[BI.p_empty + pb], ((c / NB) & 1) ^ 1);
                 tc_fence_after_sync();
                 const uint64_t dQ = smem_desc_advance(dQ0, s * L::stage_bytes), dK = smem_desc_advance(dK0, s * L::stage_bytes);
-                const uint32_t dP = tb + L::tm_p + pb * 32;
+                const uint32_t dP = tb + L::tm_p + pb * L::p_cols;
 #pragma unroll
                 for (int ks = 0; ks < DK / 16; ++ks) {
                     const uint32_t off = (ks / 4) * L::half_bytes + (ks % 4) * 32;
                     mma_bf16_ss(dP, smem_desc_advance(dQ, off), smem_desc_advance(dK, off), idP, ks > 0);
                 }
                 mma_commit(&bars[BI.p_full + pb]);
-                mma_commit_mc(&bars[BI.empty + s], kAll);
+                commit_all(&bars[BI.empty + s]);
                 TC_TRACE(1, c);
             }
         }
@@ -404,7 +420,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 }
                 mma_commit(&bars[BI.s_empty + sb]);
                 mma_commit(&bars[BI.o1_full + ob]);
-                mma_commit_mc(&bars[BI.empty + s], kAll);
+                commit_all(&bars[BI.empty + s]);
             }
         }
     } else if (warp == 4) {
@@ -427,7 +443,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                     mma_bf16_ss(dU, smem_desc_advance(dK, 2 * ks * 1024), smem_desc_advance(dV, 2 * ks * 128), idU, ks > 0);
                 mma_commit(&bars[BI.u_full + ob]);
                 mma_commit(&bars[BI.vt_empty + pb]);
-                mma_commit_mc(&bars[BI.empty + s], kAll);
+                commit_all(&bars[BI.empty + s]);
             }
         }
     } else if (warp == 5) {
@@ -454,7 +470,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                 }
                 mma_commit(&bars[BI.o2_full + ob]);
                 mma_commit(&bars[BI.vt_empty + pb]);
-                mma_commit_mc(&bars[BI.a_empty + pb], kAll);   // every CTA writes into this buffer: all of them must know
+                commit_all(&bars[BI.a_empty + pb]);   // every CTA writes into this buffer: all of them must know
             }
         }
     } else if (warp == 6 || warp == 7 || warp == 20 || warp == 21) {
@@ -529,7 +545,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             uint32_t r[NG][NA / 2];
 #pragma unroll
             for (int gi = 0; gi < NG; ++gi)
-                if (act[gi]) tmem_ld_slice<NA>(tmem_addr(tb, (C == 64) ? 32 * q : 32 * q + 16 * gi, L::tm_p + pb * 32), r[gi]);
+                if (act[gi]) tmem_ld_slice<NA>(tmem_addr(tb, (C == 64) ? 32 * q : 32 * q + 16 * gi, L::tm_p + pb * L::p_cols), r[gi]);
             tmem_ld_wait();
             tc_fence_before_sync();
             __syncwarp();
@@ -578,7 +594,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             }
             if (q == 3 && lane == 0) TC_TRACE(6, c);
             if (lane == 0) {
-                if (q == 3) mbar_arrive_expect_tx(&bars[BI.a_full + pb], tx);   // quadrant 3 holds the last rows: always active
+                if (CS > 1 && q == 3) mbar_arrive_expect_tx(&bars[BI.a_full + pb], tx);   // quadrant 3 holds the last rows: always active
                 else mbar_arrive(&bars[BI.a_full + pb]);
                 if ((c % CPB) == (uint32_t)CPB - 1 || c + 1 == n_chunks) mbar_arrive(&bars[BI.g_empty + gslot]);
             }
@@ -684,7 +700,8 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     // and no peer still multicasts, copies or arrives into this CTA once the whole cluster is here ----
     tc_fence_before_sync();
     if (threadIdx.x == 0) TC_TRACE(11, 0);
-    cluster_sync_relaxed();
+    if constexpr (CS > 1) cluster_sync_relaxed();
+    else __syncthreads();
     if (threadIdx.x == 0) TC_TRACE(12, 0);
 #ifdef ESC_TC_TRACE
     TC_TRACE_L(15, launch_id);
@@ -728,7 +745,7 @@ static int make_tmap(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, u
 template <int DK, int C, int CS, typename OutT>
 static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                        float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
-    using L = TcCfg<DK, C>;
+    using L = TcCfg<DK, C, CS>;
     static bool attr_set = false;
     if (!attr_set) {
         ESC_CUDA(cudaFuncSetAttribute(esc_scan_tc_kernel<DK, C, CS, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::total));
@@ -750,14 +767,14 @@ static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const v
     cfg.dynamicSmemBytes = L::total;
     cfg.stream = stream;
     cudaLaunchAttribute attr[2];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = CS;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.* in the kernel
-    attr[1].val.programmaticStreamSerializationAllowed = 1;
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.* in the kernel
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = CS;
+    attr[1].val.clusterDim.y = 1;
+    attr[1].val.clusterDim.z = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 2;
+    cfg.numAttrs = CS > 1 ? 2 : 1;
     ESC_CUDA(cudaLaunchKernelEx(&cfg, esc_scan_tc_kernel<DK, C, CS, OutT>, tq, tk, tv, g, state_in, state_out, (OutT*)o, s.H, s.dv, T,
                                 t_stride));
     return ESC_OK;
@@ -774,11 +791,27 @@ static int launch_tc_o(const ScanShape& s, const void* q, const void* k, const v
 // such clusters resident at this shared-memory footprint (cudaOccupancyMaxActiveClusters, r01): the 16 heads of the B = 1
 // workloads would run as two waves.  Clusters of 4 fit 33 times: 32 clusters (128 CTAs) in one wave.
 constexpr int kTcCluster = 4;
+// Short calls (the suffix scan after a restore: one or two chunks) run WITHOUT a cluster: every CTA loads whole Q / K tiles
+// and computes all C columns of P and A itself.  Per chunk that is 4x the score arithmetic and 4x the L2 -> SM traffic, but
+// a one-chunk call is a single pass through the dependent pipeline, and dropping the slice exchange and both cluster barriers
+// from it is worth more (r01, 18-layer suffix graph: 5.35 -> 4.78 us per layer at T = 64, 6.54 -> 6.20 at 128, 8.25 -> 8.48
+// at 256).  Same MMAs in the same order on the same operands: the results are bit-identical to the cluster variant's
+// (tests: restore + short suffix against the cold run).
+#ifndef ESC_TC_SHORT
+#define ESC_TC_SHORT 128
+#endif
+constexpr uint64_t kTcShortT = ESC_TC_SHORT;
 
 template <int DK, int C>
 static int launch_tc_dv(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                         float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
     if (s.dv % (kTcDVT * kTcCluster)) return ESC_ERR_UNSUPPORTED;
+    if (!state_out) {   // prepare-only call: both variants
+        const int rc = launch_tc_o<DK, C, 1>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+        if (rc != ESC_OK) return rc;
+    } else if (T <= kTcShortT) {
+        return launch_tc_o<DK, C, 1>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    }
     return launch_tc_o<DK, C, kTcCluster>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
 }
 
@@ -800,7 +833,7 @@ extern "C" int esc_debug_trace_read(long long* host) {
     return (int)cudaMemcpyFromSymbol(host, g_tc_trace, sizeof(g_tc_trace));
 }
 extern "C" int esc_debug_max_clusters(int* out8, int* out4) {
-    using L = TcCfg<128, 64>;
+    using L = TcCfg<128, 64, 4>;
     cudaLaunchConfig_t cfg = {};
     cfg.blockDim = dim3(kTcThreads);
     cfg.dynamicSmemBytes = L::total;

@@ -246,6 +246,24 @@ def test_back_to_back_scans_on_one_stream_are_ordered(esc, ctx):
         assert bits_equal(o, o_cold) and bits_equal(state, s_cold)
 
 
+def test_short_call_variant_matches_long_call_prefix_bitwise(esc, ctx):
+    # calls of up to 128 tokens run the kernel without a cluster (every CTA computes all score columns itself); longer ones
+    # in clusters of 4 that exchange score slices.  Causality makes o[:, :T] of a long call a function of the first T tokens
+    # only, so it must equal the short call's o bit for bit, ragged T included; so must the carried state at chunk multiples.
+    B, H, dk, dv, chunk, T_long = 2, 16, 128, 128, 64, 448
+    si = synth.scan_inputs(B, T_long, H, dk, dv, seed_ids=(21,), gate="slow")
+    s0 = synth.scan_state(B, H, dk, dv, seed_ids=(21,), scale=0.3)
+    dev_in = scan_dev_inputs(si)
+    s0_dev = torch.from_numpy(s0).to(DEV)
+    o_long, _, _ = run_scan(esc, ctx, dev_in, B, T_long, H, dk, dv, chunk, s0=s0_dev)
+    for T in (1, 37, 64, 100, 128):
+        o_short, s_short, _ = run_scan(esc, ctx, dev_in, B, T_long, H, dk, dv, chunk, s0=s0_dev, n=T)
+        assert bits_equal(o_short[:, :T], o_long[:, :T]), T
+        if T % chunk == 0:   # continue the long way from the short call's state: the rest of the long run, bit for bit
+            o_rest, _, _ = run_scan(esc, ctx, dev_in, B, T_long, H, dk, dv, chunk, s0=s_short, t0=T)
+            assert bits_equal(o_rest, o_long[:, T:]), T
+
+
 def test_seeded_shape_fuzz_vs_oracle(esc, ctx):
     # 24 seeded random (B, H, d_k, d_v, T, chunk, gate, S_0) combinations, ragged T included: every one within the gates,
     # every chunk-aligned restore bit-identical to its cold run
