@@ -320,14 +320,15 @@ def run_esc(args):
     sfx_alg = SUFFIX * workload.H * ALG_BYTES_PER_TOKEN_HEAD + 2 * workload.H * 128 * 128 * 4
     sfx_us = ms_suffix * 1e3 / N_LINEAR
     sfx_gbs = sfx_alg / (sfx_us * 1e-6) / 1e9
-    roof_sfx = {"kernel": "esc_scan_tc_kernel<128,64,4,float> (B1 H16 d128, T=64 suffix: one chunk per (b,h); 18 launches per step)",
+    roof_sfx = {"kernel": "esc_scan_tc_kernel<128,64,1,float> (B1 H16 d128, T=64 suffix: one chunk per (b,h); 18 launches per step)",
                 "bound": "hbm", "achieved": sfx_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": sfx_gbs / pk["hbm_gbs"],
                 "peak_source": pk["source"], "traffic": 1.89e6, "us_per_launch": sfx_us, "alg_bytes_per_launch": sfx_alg,
-                "traffic_note": "ncu r01h (profiles/r01h_suffix_scan_ncu_full.txt): dram read 1.89 MB, write 0 in the kernel's window "
+                "traffic_note": "ncu r01s (profiles/r01s_suffix_scan_ncu_full.txt): dram read 1.89 MB, write 0 in the kernel's window "
                                 "(state and outputs still dirty in L2 at kernel end)",
                 "share_of_step": ms_suffix / ms_step,
                 "note": "latency-bound by construction: 3.4 MB per launch is 0.5 us of HBM time; the launch is one chunk of "
-                        "the dependent pipeline (TMA -> P -> scores -> O2 -> store) plus setup/teardown"}
+                        "the dependent pipeline (TMA -> P -> scores -> O2 -> store) plus setup/teardown; calls of <= 128 tokens run the "
+                        "kernel without a cluster"}
     dominant = roof_sfx if ms_suffix > ms_restore + ms_snapshot else roof_copy
     out = {
         "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -23,6 +23,8 @@
 // Ring and A-buffer reuse are therefore cluster-wide events: stage / A-buffer "empty" barriers count
 // tcgen05.commit arrivals multicast from all CS CTAs.  The score path (P -> A -> O2) has its own buffers
 // (NB of each, O2 reads V from a copy the V~ warps make), so it never holds an input stage.
+// Calls of up to kTcShortT tokens use the CS = 1 instantiation instead: no cluster, every CTA loads whole Q / K tiles and
+// computes all C columns of P and A itself (bit-identical results; see kTcShortT below for why).
 // What bounds it (r01: ncu, clock64 traces, per-warp busy/wait accounting, ablation builds): the four MMA-issuing
 // threads.  They are the busiest threads of the CTA (1200-1400 of a 1400-cycle period per chunk; every other role
 // 600-1000): 28 small tcgen05.mma (M = 64, N = 16..32) and 11 tcgen05.commit per chunk at ~110 / ~130 cycles of issuing-
@@ -767,6 +769,7 @@ static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const v
     cfg.dynamicSmemBytes = L::total;
     cfg.stream = stream;
     cudaLaunchAttribute attr[2];
+    memset(attr, 0, sizeof attr);   // the value union is wider than the fields set below; stale stack bytes there changed the kernel time by 9 % (r01)
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.* in the kernel
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     attr[1].id = cudaLaunchAttributeClusterDimension;
