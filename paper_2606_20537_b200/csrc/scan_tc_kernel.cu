@@ -206,7 +206,8 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     float* gate = reinterpret_cast<float*>(sm + L::gate_off);   // [2][2][256]: b2 then eb per slot
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t rank = CS > 1 ? cluster_ctarank() : 0u;   // clusters are CS consecutive d_v slices (blockIdx.x) of one (b, h)
+    uint32_t rank = 0;
+    if constexpr (CS > 1) rank = cluster_ctarank();   // clusters are CS consecutive d_v slices (blockIdx.x) of one (b, h)
     const uint32_t bh = blockIdx.y, b = bh / H, h = bh % H, dv0 = blockIdx.x * kTcDVT;
     const uint32_t key0 = rank * NA;    // first key (= first Q / K row) of this CTA's slice
     const uint32_t n_chunks = (uint32_t)((T + C - 1) / C);
@@ -589,7 +590,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             // buffer: once the four score warps have written it, one lane per peer pushes it into the same place of that
             // peer's buffer pb; the copy completes (tx bytes) on the peer's a_full barrier
             asm volatile("bar.sync 1, 128;" ::: "memory");
-            if (q == 0 && lane < CS - 1) {
+            if constexpr (CS > 1) if (q == 0 && lane + 1 < CS) {
                 const uint32_t d = (uint32_t)lane + ((uint32_t)lane >= rank ? 1u : 0u);
                 const uint32_t off = L::a_off + pb * L::a_bytes + (key0 / 8) * L::a_lbo;
                 bulk_copy_to_cluster(mapa(sm_a + off, d), sm_a + off, kSlice, mapa(smem_u32(&bars[BI.a_full + pb]), d));

@@ -53,6 +53,8 @@ SHAPES = [
     (1, 2, 64, 64, 256, 64, "one"),         # g == 1: plain linear attention
     (1, 1, 128, 128, 1, 64, "fast"),        # T = 1
     (1, 1, 128, 128, 63, 64, "fast"),       # T < chunk
+    (2, 3, 64, 64, 128, 64, "fast"),        # two whole chunks in the cluster-free short-call variant (T <= 128), d = 64
+    (1, 2, 128, 64, 100, 128, "slow"),      # ragged second chunk in the short-call variant, d_v = 64
 ]
 
 
