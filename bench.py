@@ -8,8 +8,9 @@ a working set of capsules and L2 is flushed between timed steps (PAPER.md:301's 
 model), so neither verb reads L2-resident bytes.
 
   value  = capsule bytes moved by the verbs (snapshot r+w + restore r+w = 4 x capsule bytes) / step time, GB/s
-  e2e    = the same with the step's suffix inputs copied H2D from pinned memory and its outputs copied D2H
-           inside the timed region
+  e2e    = the same with every step's suffix inputs copied H2D from pinned memory and its outputs copied D2H inside
+           the timed region: K steps back to back, double-buffered (the copies of neighbouring steps overlap the
+           compute on their own streams); the one-step-at-a-time latency view is reported beside it (serial_*)
   extras = restore-alone GB/s, scan tokens/s at config 2's cold length, warm-vs-cold table at 2k-16k
   --impl reference times the CPU oracle (oracle/) on the same step.
 """
@@ -235,14 +236,15 @@ def run_esc(args):
             flush.fill_(1)
             flush_sink.copy_(flush.view(torch.float32).sum().reshape(1))
 
-    def step(i):
+    def step(i, g=None):
         """snapshot(P) -> ONE graph launch [restore -> 18-layer suffix scan]."""
+        g = g or graph
         j = i % N_CAPSULES
         sess.set.set_position(P_STEP)
         caps[j].destroy()
         caps[j] = esc.snapshot(sess.set, P_STEP, CHUNK, slabs[j], stream=stream)
-        graph.set_capsule(caps[(j + N_CAPSULES // 2) % N_CAPSULES], stream)   # written 10 steps ago: not in L2
-        graph.launch(stream)
+        g.set_capsule(caps[(j + N_CAPSULES // 2) % N_CAPSULES], stream)   # written 10 steps ago: not in L2
+        g.launch(stream)
         launches[0] += 2 + N_LINEAR
 
     def timed(fn, n, with_flush=True):
@@ -279,7 +281,51 @@ def run_esc(args):
             inputs.d2h()
     timed(step_e2e, 3)
     ms_e2e_l = timed(step_e2e, args.steps)
-    ms_e2e = sum(ms_e2e_l) / len(ms_e2e_l)
+    ms_e2e_serial = sum(ms_e2e_l) / len(ms_e2e_l)
+
+    # The same K steps as a user would run them back to back: two input / output buffer sets (one captured graph each), the
+    # H2D copy of step i+1 and the D2H copy of step i-1 on their own streams while step i computes.  Every step still
+    # uploads its own inputs from pinned memory and downloads its own outputs; the capsules rotate over the 20-slab
+    # working set (1.3 GiB > L2), so the copy kernels' sources are never L2-resident.  K steps are timed as one region.
+    inputs_b = workload.SuffixInputs(N_LINEAR, SUFFIX, seed=rank + 1000, device=dev, pinned=True)
+    layers_b, _ = workload.scan_layers(sess, inputs_b, CHUNK)
+    graph_b = esc.graph_capture(ctx, sess.set, P_STEP, layers_b, stream)
+    io_sets = [(inputs, graph), (inputs_b, graph_b)]
+    s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+
+    def run_pipelined(n):
+        torch.cuda.synchronize()
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev_in = [torch.cuda.Event() for _ in range(n)]
+        ev_cmp = [torch.cuda.Event() for _ in range(n)]
+        ev_out = [torch.cuda.Event() for _ in range(n)]
+        t0.record(stream)
+        s_in.wait_event(t0)
+        for i in range(n):
+            io, g = io_sets[i % 2]
+            with torch.cuda.stream(s_in):
+                if i >= 2:
+                    s_in.wait_event(ev_cmp[i - 2])        # step i-2 has consumed this input set
+                io.h2d()
+                ev_in[i].record(s_in)
+            stream.wait_event(ev_in[i])
+            if i >= 2:
+                stream.wait_event(ev_out[i - 2])          # step i-2's outputs have left this output set
+            step(i, g)
+            ev_cmp[i].record(stream)
+            with torch.cuda.stream(s_out):
+                s_out.wait_event(ev_cmp[i])
+                io.d2h()
+                ev_out[i].record(s_out)
+        stream.wait_event(ev_out[n - 1])
+        if n >= 2:
+            stream.wait_event(ev_out[n - 2])
+        t1.record(stream)
+        torch.cuda.synchronize()
+        return t0.elapsed_time(t1) / n
+    run_pipelined(max(args.warmup, 3))
+    ms_e2e = run_pipelined(args.steps)
+    graph_b.destroy()
 
     # ---- per-kernel durations (CUDA events on the launching stream, L2 flushed before each) ------------
     def only_restore(i):
@@ -304,7 +350,7 @@ def run_esc(args):
     clocks = sampler.stop()
 
     # max over ranks
-    ms_step, ms_e2e, wall_ms = max_over_ranks([ms_step, ms_e2e, wall_ms], dev)
+    ms_step, ms_e2e, ms_e2e_serial, wall_ms = max_over_ranks([ms_step, ms_e2e, ms_e2e_serial, wall_ms], dev)
     moved = 4 * payload                                  # snapshot r+w + restore r+w
     value = aggregate_value(moved, ms_step, world)
     e2e_value = aggregate_value(moved, ms_e2e, world)
@@ -342,7 +388,11 @@ def run_esc(args):
                    "value_definition": "4 x capsule bytes (snapshot r+w, restore r+w) / step time, all ranks"},
         "clocks": clocks, "gpu_launches": n_launch, "wall_ms_timed_region": wall_ms,
         "e2e": {"value": e2e_value, "unit": "GB/s", "h2d_bytes_per_step": inputs.h2d_bytes(),
-                "d2h_bytes_per_step": inputs.d2h_bytes(), "ms_per_step": ms_e2e},
+                "d2h_bytes_per_step": inputs.d2h_bytes(), "ms_per_step": ms_e2e,
+                "mode": "K steps back to back, double-buffered: H2D of step i+1 and D2H of step i-1 overlap step i "
+                        "(separate streams); every step uploads its inputs from pinned memory and downloads its outputs",
+                "serial_ms_per_step": ms_e2e_serial, "serial_value": aggregate_value(moved, ms_e2e_serial, world),
+                "serial_note": "one step at a time on one stream (H2D -> step -> D2H), L2 flushed before each: the latency view"},
         "breakdown_us": {"snapshot": ms_snapshot * 1e3, "restore": ms_restore * 1e3,
                          "suffix_scan_18_layers": ms_suffix * 1e3, "step": ms_step * 1e3},
         "restore": {"us": ms_restore * 1e3, "GBps": copy_gbs, "frac_of_measured_peak": copy_gbs / pk["hbm_gbs"],
