@@ -559,6 +559,32 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
                                                "frac_of_measured_peak": conv_alg / (conv_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
                                                "alg_bytes": "2 B read + 4 B written per element"}}
     del gin, cx, cy
+    # ---- BASELINE config 3: the 8k capsule (210 MiB) forked into 8 live sets (one launch: read once, write 8 times), then all
+    # 8 rolled back to it (8 launches) ----
+    P3, n3 = 8192, 8
+    src3 = workload.HybridSession(ctx, P3 + 128, seed=40, device=dev)
+    src3.set.set_position(P3)
+    cap3 = esc.snapshot(src3.set, P3, CHUNK, src3.new_slab(P3), stream=stream)
+    pay3 = cap3.info().payload_bytes
+    sess3 = [workload.HybridSession(ctx, P3 + 128, seed=41 + i, device=dev) for i in range(n3)]
+    sets3 = [s_.set for s_ in sess3]
+    fork_ms, _ = med_ms(lambda: esc.fork(cap3, sets3, stream=stream), n=7)
+
+    def rollback_all():
+        for s_ in sets3:
+            esc.rollback(s_, cap3, stream=stream)
+    rb_ms, _ = med_ms(rollback_all, n=7)
+    res["fork_rollback"] = {"capsule_MiB": pay3 / 2**20, "n_live_sets": n3,
+                            "fork_us": fork_ms * 1e3, "fork_GBps": (1 + n3) * pay3 / (fork_ms * 1e-3) / 1e9,
+                            "fork_frac_of_measured_peak": (1 + n3) * pay3 / (fork_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
+                            "rollback_all_us": rb_ms * 1e3, "rollback_GBps": 2 * n3 * pay3 / (rb_ms * 1e-3) / 1e9,
+                            "rollback_frac_of_measured_peak": 2 * n3 * pay3 / (rb_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
+                            "note": "BASELINE config 3 shape; algorithmic bytes: fork (1 + n) x capsule (esc_fork_kernel reads each tile "
+                                    "once and writes it n times), rollback 2 x capsule per live set (n launches of esc_copy_kernel); "
+                                    "parity: tests/test_gpu_graph.py::test_config3_fork_continue_rollback_replay"}
+    cap3.destroy()
+    del sess3, sets3, src3
+    torch.cuda.empty_cache()
     # ---- BASELINE config 4: scan sweep (B 1-4, H16, d128, T 2k-64k, chunk 64/128), device-generated inputs of the same
     # distributions (timing only; parity at these shapes is tests/test_gpu_scan.py::test_config4_sweep_points_sampled) ----
     sweep = []
