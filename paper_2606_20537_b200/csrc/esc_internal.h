@@ -131,5 +131,8 @@ struct ScanShape {
 bool decode_key(esc_shape_key key, ScanShape* s);
 int launch_scan(const esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g,
                 const float* state_in, float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream);
+// gated delta rule, chunked form on warp-level MMAs (gdn_mma_kernel.cu)
+int launch_gdn_mma(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* beta,
+                   const float* state_in, float* state_out, float* o, uint64_t T, uint64_t t_stride, cudaStream_t stream);
 
 }  // namespace esc
