@@ -6,20 +6,33 @@
 // D_ij = 2^(b_i - b_j):
 //     X_k = K S_0 , X_q = Q S_0                               (16 x d_v each)      mma  M = d_v slice, N = 16 tokens, K = d_k
 //     G_kk = K K^T , G_qk = Q K^T                             (16 x 16 each)       mma  M = 16 tokens, N = 16 tokens, K = d_k
-//     w_i = beta_i (v_i - 2^(b_i) X_k,i - sum_{j<i} D_ij G_kk,ij w_j)              16 sequential steps (rank-1 updates of
-//                                                                                   the residual, two shuffles per step)
+//     w_i = beta_i (v_i - 2^(b_i) X_k,i - sum_{j<i} D_ij G_kk,ij w_j)              sequential: rank-1 updates of the residual,
+//                                                                                   two columns per round of shuffles
 //     o_i = 2^(b_i) X_q,i + sum_{j<=i} D_ij G_qk,ij w_j                            mma  M = d_v slice, N = 16, K = 16
 //     S_16 = 2^(b_15) S_0 + sum_j 2^(b_15 - b_j) k_j^T w_j                         mma  M = d_v slice, N = d_k, K = 16
 // which is the recurrence above with the 16 updates of a chunk expanded (exact in exact arithmetic).
 //
-// Decomposition: the columns of S are independent.  ONE WARP owns (b, h, 16 columns of d_v) and keeps S^T (16 x d_k) in the
-// fp32 accumulator registers of its MMAs for the whole call: S^T is the C operand of the state update, and — re-read as an
-// A operand, a register-local relabelling of the accumulator fragments — the left factor of X^T = S^T K^T.  Every product
-// is computed transposed (d_v rows) for that reason.  fp32 factors (S, w, the decayed Gram entries) enter the bf16 MMAs as
-// two-term splits (hi + lo); q, k are the bf16 inputs themselves.  One warp per CTA: there is nothing to synchronise, and
-// B H d_v / 16 warps is all the parallelism the recurrence has.  Inputs are staged 64 tokens at a time with cp.async
-// (double buffered) into padded rows (conflict-free fragment loads).  Tokens beyond T are staged as k = q = v = 0,
-// beta = 0, a = 1: they leave the state alone.
+// Decomposition: the columns of S are independent, so one CTA owns (b, h, 16 columns of d_v).  S^T (16 x d_k) lives in the fp32
+// accumulator registers of the MMAs for the whole call: it is the C operand of the state update and — re-read as an A
+// operand, a register-local relabelling of the accumulator fragments — the left factor of X^T = S^T K^T; every product is
+// computed transposed (d_v rows) for that reason.  fp32 factors (S, w, the decayed Gram entries) enter the bf16 MMAs as
+// two-term splits (hi + lo); q, k are the bf16 inputs themselves.
+// Seven warps, by what depends on what:
+//   warps 0-3  the recurrence: each holds a quarter of d_k (of the rows of S), computes its part of X_k, X_q, exchanges the
+//              partial sums through shared memory (one named barrier per chunk, summed in warp order by every reader: same
+//              bits everywhere), solves the 16 x 16 system (redundantly: no second barrier) and updates its quarter of S;
+//              warps 0 and 1 also form o for eight tokens each;
+//   warps 4-5  the Gram matrices, decays and their products L, M: functions of the inputs only, computed one 64-token block
+//              ahead into shared memory, alternate chunks each;
+//   warp 6     cp.async loader, two blocks ahead (three input buffers, padded rows: conflict-free fragment loads).
+// One CTA barrier per block of 64 tokens hands the buffers on.  Tokens beyond T are staged as k = q = v = 0, beta = 0, a = 1:
+// they leave the state alone.
+// Bound: the per-chunk dependency chain of the recurrence warps (~1900 cycles per 16 tokens: X 230, exchange 400, residual
+// 140, solve 520, o 300, state update 180; r01 clock64 accounting), not HBM and not the tensor pipe: B H d_v / 16 = 128
+// independent chains is all the parallelism the recurrence has at B = 1.  Tried (r01): a token order that gives a lane four
+// consecutive tokens (4 rounds of shuffles instead of 8, swizzled rows against the bank conflicts it causes): slower, the
+// solve is bound by its instruction count, not by the shuffle rounds; hoisting every shared-memory load of the chain above
+// the MMAs: slower.
 //
 // Restore + continue is bit-identical to the cold run when the boundary is a multiple of 16 tokens from the start of the
 // sequence of calls (every chunk-aligned boundary is); elsewhere it agrees to rounding.
@@ -32,7 +45,9 @@ namespace esc {
 constexpr int kGmTB = 64;          // tokens per staged block
 constexpr int kGmC = 16;           // tokens per chunk
 constexpr int kGmDVT = 16;         // d_v columns per warp / CTA
-constexpr int kGmWarps = 3;         // 0: the recurrence, 1: Gram matrices one block ahead, 2: cp.async loader two blocks ahead
+constexpr int kGmRW = 4;            // recurrence warps: each owns a quarter of d_k (of the rows of S)
+constexpr int kGmGW = 2;            // Gram warps (one block ahead; the chunks of a block alternate between them)
+constexpr int kGmWarps = kGmRW + kGmGW + 1;   // + the cp.async loader (two blocks ahead)
 constexpr int kGmThreads = 32 * kGmWarps;
 constexpr int kGmNB = 3;            // staged input blocks
 
@@ -88,6 +103,7 @@ struct GmSmem {
         uint32_t Mlo[kGmC][kGmC / 2 + 1];
         float bl[kGmC];                            // inclusive cumulative log2 decay
     } ch[2][kGmTB / kGmC];
+    float4 part[2][kGmRW][4][32];                  // per chunk parity and recurrence warp: partial X_k^T (groups 0, 1 = n-tiles) and X_q^T (2, 3)
 };
 
 template <int DK>
@@ -100,17 +116,21 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
     GmSmem<DK>& sm = *reinterpret_cast<GmSmem<DK>*>(gm_raw);
     static_assert(DK == 64 || DK == 128, "d_k");
     constexpr int NKS = DK / 16, NT = DK / 8, C = kGmC;
+    constexpr int KPW = NKS / kGmRW, NTW = NT / kGmRW;   // k-steps / n-tiles of d_k per recurrence warp
+    static_assert(KPW >= 1 && NTW == 2 * KPW, "d_k split");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gq = lane >> 2, c = lane & 3;
     const uint32_t bh = blockIdx.y, b = bh / H, h = bh % H, dv0 = blockIdx.x * kGmDVT;
 
-    // S^T (16 d_v rows x d_k) in accumulator layout: St[nt][0,1] = (row gq, d_k 8nt + 2c + {0,1}), St[nt][2,3] = (row gq + 8, same)
-    float St[NT][4];
+    // S^T (16 d_v rows x d_k) in accumulator layout, the d_k range [rw DK/4, (rw+1) DK/4) of it in recurrence warp rw:
+    // St[l][0,1] = (row gq, d_k 8 (rw NTW + l) + 2c + {0,1}), St[l][2,3] = (row gq + 8, same)
+    const int rw = warp < kGmRW ? warp : 0;
+    float St[NTW][4];
 #pragma unroll
-    for (int nt = 0; nt < NT; ++nt) {
+    for (int l = 0; l < NTW; ++l) {
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            const size_t dk = 8 * nt + 2 * c + (e & 1), dv = dv0 + gq + 8 * (e >> 1);
-            St[nt][e] = (warp == 0 && state_in) ? state_in[((size_t)bh * DK + dk) * DV + dv] : 0.f;
+            const size_t dk = 8 * (rw * NTW + l) + 2 * c + (e & 1), dv = dv0 + gq + 8 * (e >> 1);
+            St[l][e] = (warp < kGmRW && state_in) ? state_in[((size_t)bh * DK + dk) * DV + dv] : 0.f;
         }
     }
 
@@ -205,16 +225,18 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
         }
     };
     // ---- recurrence warp: one chunk of the carry chain ----
+    uint32_t chunk_no = 0;   // running chunk count (the parity picks the partial-sum buffer)
     auto main_chunk = [&](int buf, int c0, const typename GmSmem<DK>::Chunk& ck, uint64_t t0, int n) {
-        // X_k^T, X_q^T (d_v x tokens); the hi and lo terms of S accumulate separately (independent MMA chains)
+        // partial X_k^T, X_q^T (d_v x tokens) over this warp's quarter of d_k; hi and lo terms of S accumulate separately
         float xk[2][4] = {}, xq[2][4] = {}, xkl[2][4] = {}, xql[2][4] = {};
 #pragma unroll
-        for (int ks = 0; ks < NKS; ++ks) {
+        for (int kl = 0; kl < KPW; ++kl) {
+            const int ks = rw * KPW + kl;
             uint32_t ah[4], al[4];
-            ah[0] = gm_split(St[2 * ks][0], St[2 * ks][1], al[0]);
-            ah[1] = gm_split(St[2 * ks][2], St[2 * ks][3], al[1]);
-            ah[2] = gm_split(St[2 * ks + 1][0], St[2 * ks + 1][1], al[2]);
-            ah[3] = gm_split(St[2 * ks + 1][2], St[2 * ks + 1][3], al[3]);
+            ah[0] = gm_split(St[2 * kl][0], St[2 * kl][1], al[0]);
+            ah[1] = gm_split(St[2 * kl][2], St[2 * kl][3], al[1]);
+            ah[2] = gm_split(St[2 * kl + 1][0], St[2 * kl + 1][1], al[2]);
+            ah[3] = gm_split(St[2 * kl + 1][2], St[2 * kl + 1][3], al[3]);
 #pragma unroll
             for (int nt = 0; nt < 2; ++nt) {
                 const __nv_bfloat16* kr = &sm.k[buf][c0 + 8 * nt + gq][16 * ks + 2 * c];
@@ -227,13 +249,36 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
                 gm_mma(xql[nt], al, bq0, bq1);
             }
         }
+        // exchange: every recurrence warp needs the whole X_k; warps 0 and 1 the X_q of the eight tokens they write o for.
+        // Summed in warp order by every reader: the same bits everywhere.
+        {
+            float4(*pb)[4][32] = sm.part[chunk_no & 1];
 #pragma unroll
-        for (int nt = 0; nt < 2; ++nt) {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                xk[nt][e] += xkl[nt][e];
-                xq[nt][e] += xql[nt][e];
+            for (int nt = 0; nt < 2; ++nt) {
+                pb[rw][nt][lane] = make_float4(xk[nt][0] + xkl[nt][0], xk[nt][1] + xkl[nt][1], xk[nt][2] + xkl[nt][2], xk[nt][3] + xkl[nt][3]);
+                pb[rw][2 + nt][lane] = make_float4(xq[nt][0] + xql[nt][0], xq[nt][1] + xql[nt][1], xq[nt][2] + xql[nt][2], xq[nt][3] + xql[nt][3]);
             }
+            asm volatile("bar.sync 1, %0;" ::"n"(32 * kGmRW) : "memory");
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) {
+                float4 sk = pb[0][nt][lane];
+#pragma unroll
+                for (int w2 = 1; w2 < kGmRW; ++w2) {
+                    const float4 t = pb[w2][nt][lane];
+                    sk.x += t.x; sk.y += t.y; sk.z += t.z; sk.w += t.w;
+                }
+                xk[nt][0] = sk.x; xk[nt][1] = sk.y; xk[nt][2] = sk.z; xk[nt][3] = sk.w;
+                if (nt == rw) {   // X_q only where this warp writes o
+                    float4 sq = pb[0][2 + nt][lane];
+#pragma unroll
+                    for (int w2 = 1; w2 < kGmRW; ++w2) {
+                        const float4 t = pb[w2][2 + nt][lane];
+                        sq.x += t.x; sq.y += t.y; sq.z += t.z; sq.w += t.w;
+                    }
+                    xq[nt][0] = sq.x; xq[nt][1] = sq.y; xq[nt][2] = sq.z; xq[nt][3] = sq.w;
+                }
+            }
+            ++chunk_no;
         }
         // ---- residual R^T = V^T - 2^(b) X_k^T in accumulator layout: r[nt][e] = (row gq, token 8nt + 2c + e), r[nt][2+e] = row gq + 8 ----
         float r[2][4], eb[2][2], bt[2][2];
@@ -249,21 +294,28 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
             }
         }
         // ---- the 16 x 16 unit-triangular system, right-looking: r_j -= (beta_i L_ji) r_i for j > i, then w = beta r.  Column i
-        // lives in the lanes with c = (i % 8) / 2: two shuffles broadcast it inside each 4-lane group.  L is zero on and
-        // above the diagonal, so the update can run over every column a lane holds. ----
+        // lives in the lanes with c = (i % 8) / 2: shuffles broadcast it inside each 4-lane group.  L is zero on and above
+        // the diagonal, so the update can run over every column a lane holds. ----
 #pragma unroll
-        for (int i = 0; i < C; ++i) {
-            const int nti = i >> 3, ci = (i & 7) >> 1, ei = i & 1;
-            const float wv0 = __shfl_sync(0xffffffffu, r[nti][ei], (lane & ~3) | ci);
-            const float wv1 = __shfl_sync(0xffffffffu, r[nti][2 + ei], (lane & ~3) | ci);
+        for (int pr = 0; pr < C / 2; ++pr) {
+            // columns i0 = 2 pr and i0 + 1 sit in the same lanes (c = pr % 4): the owner finishes column i0 + 1 itself, then both
+            // columns are broadcast in one round of shuffles: 8 dependent rounds instead of 16
+            const int i0c = 2 * pr, nti = pr >> 2, ci = pr & 3;
+            const float l10 = ck.L[i0c + 1][i0c];
+            const float a0 = r[nti][0], a1 = r[nti][2];
+            const float b0 = fmaf(-l10, a0, r[nti][1]), b1 = fmaf(-l10, a1, r[nti][3]);
+            const int src = (lane & ~3) | ci;
+            const float wa0 = __shfl_sync(0xffffffffu, a0, src), wa1 = __shfl_sync(0xffffffffu, a1, src);
+            const float wb0 = __shfl_sync(0xffffffffu, b0, src), wb1 = __shfl_sync(0xffffffffu, b1, src);
 #pragma unroll
             for (int nt = 0; nt < 2; ++nt) {
-                if (8 * nt + 7 <= i) continue;   // every column of this n-tile is <= i: nothing below the diagonal
+                if (8 * nt + 7 <= i0c) continue;   // every column of this n-tile is <= i0: nothing below the diagonal
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
-                    const float lji = ck.L[8 * nt + 2 * c + e][i];
-                    r[nt][e] = fmaf(-lji, wv0, r[nt][e]);
-                    r[nt][2 + e] = fmaf(-lji, wv1, r[nt][2 + e]);
+                    const int j = 8 * nt + 2 * c + e;
+                    const float lja = ck.L[j][i0c], ljb = ck.L[j][i0c + 1];   // zero on and above the diagonal
+                    r[nt][e] = fmaf(-ljb, wb0, fmaf(-lja, wa0, r[nt][e]));
+                    r[nt][2 + e] = fmaf(-ljb, wb1, fmaf(-lja, wa1, r[nt][2 + e]));
                 }
             }
         }
@@ -285,12 +337,16 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
             wh[3] = gm_split(w[1][2], w[1][3], wl[3]);
 #pragma unroll
             for (int nt = 0; nt < 2; ++nt) {
+                if (nt != rw) continue;   // warp 0 writes o of tokens 0-7 of the chunk, warp 1 of tokens 8-15
                 float oa[4] = {0.f, 0.f, 0.f, 0.f};
                 const uint32_t mh0 = ck.Mhi[8 * nt + gq][c], mh1 = ck.Mhi[8 * nt + gq][4 + c];
                 const uint32_t ml0 = ck.Mlo[8 * nt + gq][c], ml1 = ck.Mlo[8 * nt + gq][4 + c];
+                float ob[4] = {0.f, 0.f, 0.f, 0.f}, oc[4] = {0.f, 0.f, 0.f, 0.f};
                 gm_mma(oa, wh, mh0, mh1);
-                gm_mma(oa, wl, mh0, mh1);
-                gm_mma(oa, wh, ml0, ml1);
+                gm_mma(ob, wl, mh0, mh1);
+                gm_mma(oc, wh, ml0, ml1);
+#pragma unroll
+                for (int e = 0; e < 4; ++e) oa[e] += ob[e] + oc[e];
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int j = 8 * nt + 2 * c + e;
@@ -321,46 +377,48 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
             wh[2] = gm_split(ws[1][0], ws[1][1], wl[2]);
             wh[3] = gm_split(ws[1][2], ws[1][3], wl[3]);
 #pragma unroll
-            for (int p = 0; p < NT / 2; ++p) {
+            for (int pl = 0; pl < NTW / 2; ++pl) {
+                const int p = rw * (NTW / 2) + pl;
                 uint32_t kb[4];
                 // matrix m = lane / 8: rows = tokens 8 (m % 2) + lane % 8, columns = d_k 16 p + 8 (m / 2) ..
                 gm_ldmatrix_x4_trans(kb, &sm.k[buf][c0 + 8 * ((lane >> 3) & 1) + (lane & 7)][16 * p + 8 * (lane >> 4)]);
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    St[2 * p][e] *= gam;
-                    St[2 * p + 1][e] *= gam;
+                    St[2 * pl][e] *= gam;
+                    St[2 * pl + 1][e] *= gam;
                 }
-                gm_mma(St[2 * p], wh, kb[0], kb[1]);
-                gm_mma(St[2 * p + 1], wh, kb[2], kb[3]);
-                gm_mma(St[2 * p], wl, kb[0], kb[1]);
-                gm_mma(St[2 * p + 1], wl, kb[2], kb[3]);
+                gm_mma(St[2 * pl], wh, kb[0], kb[1]);
+                gm_mma(St[2 * pl + 1], wh, kb[2], kb[3]);
+                gm_mma(St[2 * pl], wl, kb[0], kb[1]);
+                gm_mma(St[2 * pl + 1], wl, kb[2], kb[3]);
             }
         }
     };
 
     // ---- block pipeline: in period p the loader stages block p + 2, the Gram warp works on block p + 1, the recurrence on block p;
     // one CTA barrier per period (64 tokens) is all the synchronisation there is ----
-    if (warp == 2) {
+    if (warp == kGmRW + kGmGW) {
         if (n_blocks > 0) stage(0, 0);
         if (n_blocks > 1) stage(1, 1);
         gm_cp_wait<0>();
     }
     __syncthreads();
-    if (warp == 1 && n_blocks > 0) {
+    const int gw = warp - kGmRW;   // Gram warp index (valid for the Gram warps only)
+    if (gw >= 0 && gw < kGmGW && n_blocks > 0) {
         const int n0 = (int)(T < (uint64_t)kGmTB ? T : (uint64_t)kGmTB);
-        for (int c0 = 0; c0 < n0; c0 += C) gram_chunk(0, c0, sm.ch[0][c0 / C]);
+        for (int c0 = gw * C; c0 < n0; c0 += kGmGW * C) gram_chunk(0, c0, sm.ch[0][c0 / C]);
     }
     __syncthreads();
     for (uint64_t blk = 0; blk < n_blocks; ++blk) {
         const uint64_t t0 = blk * kGmTB;
         const int n = (int)((T - t0) < (uint64_t)kGmTB ? (T - t0) : (uint64_t)kGmTB);
-        if (warp == 0) {
+        if (warp < kGmRW) {
             for (int c0 = 0; c0 < n; c0 += C) main_chunk((int)(blk % kGmNB), c0, sm.ch[blk & 1][c0 / C], t0, n);
-        } else if (warp == 1) {
+        } else if (gw < kGmGW) {
             if (blk + 1 < n_blocks) {
                 const uint64_t t1 = t0 + kGmTB;
                 const int n1 = (int)((T - t1) < (uint64_t)kGmTB ? (T - t1) : (uint64_t)kGmTB);
-                for (int c0 = 0; c0 < n1; c0 += C) gram_chunk((int)((blk + 1) % kGmNB), c0, sm.ch[(blk + 1) & 1][c0 / C]);
+                for (int c0 = gw * C; c0 < n1; c0 += kGmGW * C) gram_chunk((int)((blk + 1) % kGmNB), c0, sm.ch[(blk + 1) & 1][c0 / C]);
             }
         } else {
             if (blk + 2 < n_blocks) {
@@ -370,13 +428,13 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
         }
         __syncthreads();
     }
-    if (warp != 0) return;
+    if (warp >= kGmRW) return;
 #pragma unroll
-    for (int nt = 0; nt < NT; ++nt) {
+    for (int l = 0; l < NTW; ++l) {
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            const size_t dk = 8 * nt + 2 * c + (e & 1), dv = dv0 + gq + 8 * (e >> 1);
-            state_out[((size_t)bh * DK + dk) * DV + dv] = St[nt][e];
+            const size_t dk = 8 * (rw * NTW + l) + 2 * c + (e & 1), dv = dv0 + gq + 8 * (e >> 1);
+            state_out[((size_t)bh * DK + dk) * DV + dv] = St[l][e];
         }
     }
 }
