@@ -39,7 +39,7 @@ def parse_args():
     ap.add_argument("--impl", default="esc", choices=["esc", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the scan / warm-vs-cold / cpu_baseline extras")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--profile", default=None, choices=["scan", "restore", "suffix"],
+    ap.add_argument("--profile", default=None, choices=["scan", "restore", "suffix", "gdn"],
                     help="ncu driver: launch only the cold 16448-token scan (x3), only the 66 MiB restore (x5) or only the 18 "
                          "64-token suffix scans (x2); no JSON line")
     return ap.parse_args()
@@ -625,6 +625,15 @@ def run_profile(args):
         key = esc.shape_key_make(1, 16, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
         for _ in range(3):
             esc.linattn_scan(ctx, key, *full.dev[0], None, sess.states[0], full.out[0], T, T, CHUNK, stream=stream)
+    elif args.profile == "gdn":
+        from paper_2606_20537_b200 import synth
+        T = 16384 + SUFFIX
+        sess = workload.HybridSession(ctx, 64, seed=7)
+        full = workload.SuffixInputs(1, T, seed=11)
+        beta = torch.from_numpy(synth.gdn_beta(workload.B, T, workload.H, seed_ids=(11,))).to("cuda:0")
+        key = esc.shape_key_make(1, 16, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
+        for _ in range(3):
+            esc.gdn_scan(ctx, key, *full.dev[0], beta, None, sess.states[0], full.out[0], T, T, stream=stream)
     elif args.profile == "suffix":
         sess = workload.HybridSession(ctx, P_STEP + SUFFIX, seed=0)
         inputs = workload.SuffixInputs(N_LINEAR, SUFFIX, seed=0)
