@@ -17,14 +17,16 @@
 // operand, a register-local relabelling of the accumulator fragments — the left factor of X^T = S^T K^T; every product is
 // computed transposed (d_v rows) for that reason.  fp32 factors (S, w, the decayed Gram entries) enter the bf16 MMAs as
 // two-term splits (hi + lo); q, k are the bf16 inputs themselves.
-// Seven warps, by what depends on what:
+// Nine warps, by what depends on what:
 //   warps 0-3  the recurrence: each holds a quarter of d_k (of the rows of S), computes its part of X_k, X_q, exchanges the
 //              partial sums through shared memory (one named barrier per chunk, summed in warp order by every reader: same
 //              bits everywhere), solves the 16 x 16 system (redundantly: no second barrier) and updates its quarter of S;
-//              warps 0 and 1 also form o for eight tokens each;
+//              warp 0 leaves W of the chunk in a shared-memory slot for the output warps;
 //   warps 4-5  the Gram matrices, decays and their products L, M: functions of the inputs only, computed one 64-token block
 //              ahead into shared memory, alternate chunks each;
-//   warp 6     cp.async loader, two blocks ahead (three input buffers, padded rows: conflict-free fragment loads).
+//   warp 6     cp.async loader, two blocks ahead (three input buffers, padded rows: conflict-free fragment loads);
+//   warps 7-8  the outputs, off the carry chain: o of eight tokens of each chunk from the partial X_q, W and M (named
+//              full / empty barriers per chunk parity; the recurrence runs up to two chunks ahead of them).
 // One CTA barrier per block of 64 tokens hands the buffers on.  Tokens beyond T are staged as k = q = v = 0, beta = 0, a = 1:
 // they leave the state alone.
 // Bound: the per-chunk dependency chain of the recurrence warps (~1900 cycles per 16 tokens: X 230, exchange 400, residual
@@ -47,7 +49,8 @@ constexpr int kGmC = 16;           // tokens per chunk
 constexpr int kGmDVT = 16;         // d_v columns per warp / CTA
 constexpr int kGmRW = 4;            // recurrence warps: each owns a quarter of d_k (of the rows of S)
 constexpr int kGmGW = 2;            // Gram warps (one block ahead; the chunks of a block alternate between them)
-constexpr int kGmWarps = kGmRW + kGmGW + 1;   // + the cp.async loader (two blocks ahead)
+constexpr int kGmOW = 2;            // output warps: o of eight tokens of each chunk, one chunk behind the recurrence
+constexpr int kGmWarps = kGmRW + kGmGW + 1 + kGmOW;   // + the cp.async loader (two blocks ahead)
 constexpr int kGmThreads = 32 * kGmWarps;
 constexpr int kGmNB = 3;            // staged input blocks
 
@@ -89,6 +92,12 @@ __device__ __forceinline__ void gm_ldmatrix_x4_trans(uint32_t (&r)[4], const voi
                  : "r"((uint32_t)__cvta_generic_to_shared(row_ptr)));
 }
 
+__device__ __forceinline__ void gm_bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void gm_bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+// named barriers: 1 = the recurrence warps' exchange; 2, 3 = "W of the chunk is in its slot" (per chunk parity: recurrence warp 0
+// arrives, the output warps wait); 4, 5 = "slot and partial sums of that parity consumed" (output warps arrive, recurrence warps wait)
+constexpr int kGmBarFull = 2, kGmBarEmpty = 4;
+
 template <int DK>
 struct GmSmem {
     static constexpr int KS = DK + 8;              // padded row (bf16 elements): fragment loads hit 32 distinct banks
@@ -103,6 +112,7 @@ struct GmSmem {
         uint32_t Mlo[kGmC][kGmC / 2 + 1];
         float bl[kGmC];                            // inclusive cumulative log2 decay
     } ch[2][kGmTB / kGmC];
+    float4 wslot[2][2][32];                        // per chunk parity: W^T of the chunk in accumulator layout (8 values per lane)
     float4 part[2][kGmRW][4][32];                  // per chunk parity and recurrence warp: partial X_k^T (groups 0, 1 = n-tiles) and X_q^T (2, 3)
 };
 
@@ -226,7 +236,11 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
     };
     // ---- recurrence warp: one chunk of the carry chain ----
     uint32_t chunk_no = 0;   // running chunk count (the parity picks the partial-sum buffer)
-    auto main_chunk = [&](int buf, int c0, const typename GmSmem<DK>::Chunk& ck, uint64_t t0, int n) {
+    const uint32_t total_chunks = (uint32_t)((T + C - 1) / C);
+    auto main_chunk = [&](int buf, int c0, const typename GmSmem<DK>::Chunk& ck) {
+        const int par = (int)(chunk_no & 1);
+        // the output warps are done with the partial sums and the W slot of chunk_no - 2
+        if (chunk_no >= 2) gm_bar_sync(kGmBarEmpty + par, 32 * (kGmRW + kGmOW));
         // partial X_k^T, X_q^T (d_v x tokens) over this warp's quarter of d_k; hi and lo terms of S accumulate separately
         float xk[2][4] = {}, xq[2][4] = {}, xkl[2][4] = {}, xql[2][4] = {};
 #pragma unroll
@@ -249,8 +263,8 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
                 gm_mma(xql[nt], al, bq0, bq1);
             }
         }
-        // exchange: every recurrence warp needs the whole X_k; warps 0 and 1 the X_q of the eight tokens they write o for.
-        // Summed in warp order by every reader: the same bits everywhere.
+        // exchange: every recurrence warp needs the whole X_k (summed in warp order by every reader: the same bits everywhere);
+        // the partial X_q are summed by the output warps
         {
             float4(*pb)[4][32] = sm.part[chunk_no & 1];
 #pragma unroll
@@ -268,17 +282,7 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
                     sk.x += t.x; sk.y += t.y; sk.z += t.z; sk.w += t.w;
                 }
                 xk[nt][0] = sk.x; xk[nt][1] = sk.y; xk[nt][2] = sk.z; xk[nt][3] = sk.w;
-                if (nt == rw) {   // X_q only where this warp writes o
-                    float4 sq = pb[0][2 + nt][lane];
-#pragma unroll
-                    for (int w2 = 1; w2 < kGmRW; ++w2) {
-                        const float4 t = pb[w2][2 + nt][lane];
-                        sq.x += t.x; sq.y += t.y; sq.z += t.z; sq.w += t.w;
-                    }
-                    xq[nt][0] = sq.x; xq[nt][1] = sq.y; xq[nt][2] = sq.z; xq[nt][3] = sq.w;
-                }
             }
-            ++chunk_no;
         }
         // ---- residual R^T = V^T - 2^(b) X_k^T in accumulator layout: r[nt][e] = (row gq, token 8nt + 2c + e), r[nt][2+e] = row gq + 8 ----
         float r[2][4], eb[2][2], bt[2][2];
@@ -328,35 +332,11 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
                 w[nt][2 + e] = bt[nt][e] * r[nt][2 + e];
             }
         }
-        // ---- o^T = 2^(b) X_q^T + W^T M^T  (A = W^T from the registers above, B from M in shared memory) ----
-        {
-            uint32_t wh[4], wl[4];
-            wh[0] = gm_split(w[0][0], w[0][1], wl[0]);
-            wh[1] = gm_split(w[0][2], w[0][3], wl[1]);
-            wh[2] = gm_split(w[1][0], w[1][1], wl[2]);
-            wh[3] = gm_split(w[1][2], w[1][3], wl[3]);
-#pragma unroll
-            for (int nt = 0; nt < 2; ++nt) {
-                if (nt != rw) continue;   // warp 0 writes o of tokens 0-7 of the chunk, warp 1 of tokens 8-15
-                float oa[4] = {0.f, 0.f, 0.f, 0.f};
-                const uint32_t mh0 = ck.Mhi[8 * nt + gq][c], mh1 = ck.Mhi[8 * nt + gq][4 + c];
-                const uint32_t ml0 = ck.Mlo[8 * nt + gq][c], ml1 = ck.Mlo[8 * nt + gq][4 + c];
-                float ob[4] = {0.f, 0.f, 0.f, 0.f}, oc[4] = {0.f, 0.f, 0.f, 0.f};
-                gm_mma(oa, wh, mh0, mh1);
-                gm_mma(ob, wl, mh0, mh1);
-                gm_mma(oc, wh, ml0, ml1);
-#pragma unroll
-                for (int e = 0; e < 4; ++e) oa[e] += ob[e] + oc[e];
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int j = 8 * nt + 2 * c + e;
-                    if (c0 + j < n) {
-                        float* op = o + (((size_t)b * t_stride + t0 + c0 + j) * H + h) * DV + dv0;
-                        op[gq] = fmaf(eb[nt][e], xq[nt][e], oa[e]);
-                        op[gq + 8] = fmaf(eb[nt][e], xq[nt][2 + e], oa[2 + e]);
-                    }
-                }
-            }
+        // ---- hand W^T to the output warps (every recurrence warp holds the same W: warp 0 writes it) ----
+        if (rw == 0) {
+            sm.wslot[par][0][lane] = make_float4(w[0][0], w[0][1], w[0][2], w[0][3]);
+            sm.wslot[par][1][lane] = make_float4(w[1][0], w[1][1], w[1][2], w[1][3]);
+            gm_bar_arrive(kGmBarFull + par, 32 * (1 + kGmOW));
         }
         // ---- S^T <- 2^(b_15) S^T + (2^(b_15 - b_j) w_j)^T K  (B fragments of K by transposing ldmatrix) ----
         {
@@ -393,6 +373,43 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
                 gm_mma(St[2 * pl + 1], wl, kb[2], kb[3]);
             }
         }
+        ++chunk_no;
+    };
+    // ---- output warp ow: o of tokens 8 ow .. 8 ow + 7 of the chunk:  o^T = 2^(b) X_q^T + W^T M^T ----
+    auto out_chunk = [&](int buf, int c0, const typename GmSmem<DK>::Chunk& ck, uint64_t t0, int n, int nt) {
+        const int par = (int)(chunk_no & 1);
+        gm_bar_sync(kGmBarFull + par, 32 * (1 + kGmOW));
+        const float4 w0 = sm.wslot[par][0][lane], w1 = sm.wslot[par][1][lane];
+        float4 sq = sm.part[par][0][2 + nt][lane];
+#pragma unroll
+        for (int w2 = 1; w2 < kGmRW; ++w2) {
+            const float4 t = sm.part[par][w2][2 + nt][lane];
+            sq.x += t.x; sq.y += t.y; sq.z += t.z; sq.w += t.w;
+        }
+        if (chunk_no + 2 < total_chunks) gm_bar_arrive(kGmBarEmpty + par, 32 * (kGmRW + kGmOW));   // slot and partial sums read
+        const float xq[4] = {sq.x, sq.y, sq.z, sq.w};
+        uint32_t wh[4], wl[4];
+        wh[0] = gm_split(w0.x, w0.y, wl[0]);
+        wh[1] = gm_split(w0.z, w0.w, wl[1]);
+        wh[2] = gm_split(w1.x, w1.y, wl[2]);
+        wh[3] = gm_split(w1.z, w1.w, wl[3]);
+        const uint32_t mh0 = ck.Mhi[8 * nt + gq][c], mh1 = ck.Mhi[8 * nt + gq][4 + c];
+        const uint32_t ml0 = ck.Mlo[8 * nt + gq][c], ml1 = ck.Mlo[8 * nt + gq][4 + c];
+        float oa[4] = {0.f, 0.f, 0.f, 0.f}, ob[4] = {0.f, 0.f, 0.f, 0.f}, oc[4] = {0.f, 0.f, 0.f, 0.f};
+        gm_mma(oa, wh, mh0, mh1);
+        gm_mma(ob, wl, mh0, mh1);
+        gm_mma(oc, wh, ml0, ml1);
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int j = 8 * nt + 2 * c + e;
+            if (c0 + j < n) {
+                const float ebj = gm_ex2(ck.bl[j]);
+                float* op = o + (((size_t)b * t_stride + t0 + c0 + j) * H + h) * DV + dv0;
+                op[gq] = fmaf(ebj, xq[e], oa[e] + (ob[e] + oc[e]));
+                op[gq + 8] = fmaf(ebj, xq[2 + e], oa[2 + e] + (ob[2 + e] + oc[2 + e]));
+            }
+        }
+        ++chunk_no;
     };
 
     // ---- block pipeline: in period p the loader stages block p + 2, the Gram warp works on block p + 1, the recurrence on block p;
@@ -413,7 +430,10 @@ __global__ void __launch_bounds__(kGmThreads) esc_gdn_mma_kernel(const __nv_bflo
         const uint64_t t0 = blk * kGmTB;
         const int n = (int)((T - t0) < (uint64_t)kGmTB ? (T - t0) : (uint64_t)kGmTB);
         if (warp < kGmRW) {
-            for (int c0 = 0; c0 < n; c0 += C) main_chunk((int)(blk % kGmNB), c0, sm.ch[blk & 1][c0 / C], t0, n);
+            for (int c0 = 0; c0 < n; c0 += C) main_chunk((int)(blk % kGmNB), c0, sm.ch[blk & 1][c0 / C]);
+        } else if (warp > kGmRW + kGmGW) {
+            for (int c0 = 0; c0 < n; c0 += C)
+                out_chunk((int)(blk % kGmNB), c0, sm.ch[blk & 1][c0 / C], t0, n, warp - (kGmRW + kGmGW + 1));
         } else if (gw < kGmGW) {
             if (blk + 1 < n_blocks) {
                 const uint64_t t1 = t0 + kGmTB;
