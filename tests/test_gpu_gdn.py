@@ -54,7 +54,7 @@ def test_gdn_vs_oracle(esc, ctx, B, H, dk, dv, T, gate, with_s0):
     o_ref, s_ref = oracle.gdn_recurrence(q, k, v, g, beta, None if s0 is None else s0.astype(np.float64))
     assert err_o(o.cpu().numpy(), o_ref) <= TOL_O
     assert err_s(s.cpu().numpy(), s_ref) <= TOL_S
-    assert err_o(o.cpu().numpy(), o_ref) <= 1e-5 and err_s(s.cpu().numpy(), s_ref) <= 1e-5   # fp32 path: far inside the gates
+    assert err_o(o.cpu().numpy(), o_ref) <= 5e-5 and err_s(s.cpu().numpy(), s_ref) <= 5e-5   # two-term bf16 operands, fp32 accumulation: far inside the gates
 
 
 def test_gdn_restore_continue_bit_identical_at_chunk_boundaries(esc, ctx):
