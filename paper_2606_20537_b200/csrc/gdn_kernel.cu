@@ -11,27 +11,44 @@ namespace esc {
 // ---- short causal depthwise convolution, window W <= 8 -----------------------------------------------------
 // Bound: HBM (2 B read + 4 B written per element).  A thread owns 4 consecutive channels (one 8-byte bf16 vector; a
 // warp reads 256 contiguous bytes of a token row) and walks kConvRun consecutive tokens with the W-1 previous input
-// vectors and its 8 x W taps in registers, so every input vector is loaded once per run (+ W-1 to prime the window).
+// vectors and its 4 x W taps in registers, so every input vector is loaded once per run (+ W-1 to prime the window).
+// The loads are software-pipelined: the kConvU vectors of the next batch are issued (L1 no-allocate) before the current
+// batch is computed and stored, so a thread always has a batch in flight (r01u: 150 -> 113 us at 16 448 x 6144, W = 4;
+// without the pipelining the loop is issue -> wait -> compute -> store and the SM's bytes in flight drop between batches).
+// SiLU is s / (1 + e^-s) with ex2.approx and the approximate divide (2 ulp each; the full-precision expf + IEEE divide
+// made the kernel ALU-bound: 150 -> 120 us on their own); for s < -88 the quotient is -0 where the exact value is ~ -1e-37.
 constexpr int kConvMaxW = 8;
 constexpr int kConvRun = 64;      // tokens per thread
 constexpr int kConvThreads = 128;
 constexpr int kConvCPT = 4;       // channels per thread (8-byte bf16 vectors: a warp reads 256 contiguous bytes of a token row)
+constexpr int kConvU = 4;         // vectors per batch (one batch in flight per thread while the previous one is computed)
 
 __device__ __forceinline__ void bf16x4_to_f32(const uint2& raw, float (&x)[4]) {
     x[0] = __uint_as_float(raw.x << 16); x[1] = __uint_as_float(raw.x & 0xFFFF0000u);
     x[2] = __uint_as_float(raw.y << 16); x[3] = __uint_as_float(raw.y & 0xFFFF0000u);
+}
+__device__ __forceinline__ uint2 ld_stream8(const __nv_bfloat16* p) {
+    uint2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "l"(p));
+    return r;
 }
 
 template <int W>
 __global__ void __launch_bounds__(kConvThreads) esc_causal_conv_kernel(const __nv_bfloat16* __restrict__ x, const float* __restrict__ w,
                                                                        const float* __restrict__ state_in, float* __restrict__ y,
                                                                        uint64_t T, uint64_t t_stride, uint32_t C, uint32_t silu) {
-    constexpr int P = kConvCPT;
+    constexpr int P = kConvCPT, U = kConvU;
     const uint32_t cg = blockIdx.x * kConvThreads + threadIdx.x;   // channel group
     if (cg >= C / P) return;
     const uint32_t b = blockIdx.z;
     const uint64_t t_begin = (uint64_t)blockIdx.y * kConvRun;
-    const uint64_t t_end = t_begin + kConvRun < T ? t_begin + kConvRun : T;
+    const uint32_t n_tok = (uint32_t)(t_begin + kConvRun < T ? kConvRun : T - t_begin);
+    const __nv_bfloat16* xp = x + ((size_t)b * t_stride + t_begin) * C + cg * P;
+    float* yp = y + ((size_t)b * T + t_begin) * C + cg * P;
+    uint2 nxt[U];   // the batch in flight
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+        if ((uint32_t)u < n_tok) nxt[u] = ld_stream8(xp + (size_t)u * C);
     float wt[W][P];   // wt[i][j] = tap i of channel P cg + j
 #pragma unroll
     for (int j = 0; j < P; ++j)
@@ -43,24 +60,23 @@ __global__ void __launch_bounds__(kConvThreads) esc_causal_conv_kernel(const __n
     for (int i = 0; i < W - 1; ++i) {
         const int64_t s = (int64_t)t_begin - (W - 1) + i;
         if (s >= 0) {
-            bf16x4_to_f32(*reinterpret_cast<const uint2*>(x + ((size_t)b * t_stride + (uint64_t)s) * C + cg * P), win[i]);
+            bf16x4_to_f32(ld_stream8(x + ((size_t)b * t_stride + (uint64_t)s) * C + cg * P), win[i]);
         } else {
 #pragma unroll
             for (int j = 0; j < P; ++j)
                 win[i][j] = state_in ? state_in[((size_t)b * C + cg * P + j) * (W - 1) + (uint32_t)((int64_t)(W - 1) + s)] : 0.f;
         }
     }
-    const __nv_bfloat16* xp = x + ((size_t)b * t_stride + t_begin) * C + cg * P;
-    float* yp = y + ((size_t)b * T + t_begin) * C + cg * P;
-    constexpr int U = 4;   // loads in flight per thread
-    for (uint64_t t = t_begin; t < t_end; t += U) {
+    for (uint32_t t = 0; t < n_tok; t += U) {
         uint2 raw[U];
 #pragma unroll
+        for (int u = 0; u < U; ++u) raw[u] = nxt[u];
+#pragma unroll
         for (int u = 0; u < U; ++u)
-            if (t + u < t_end) raw[u] = *reinterpret_cast<const uint2*>(xp + (size_t)u * C);
+            if (t + U + u < n_tok) nxt[u] = ld_stream8(xp + (size_t)(U + u) * C);
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            if (t + u < t_end) {
+            if (t + u < n_tok) {
                 bf16x4_to_f32(raw[u], win[W - 1]);
                 float acc[P];
 #pragma unroll
@@ -68,7 +84,7 @@ __global__ void __launch_bounds__(kConvThreads) esc_causal_conv_kernel(const __n
                     float s_ = 0.f;
 #pragma unroll
                     for (int i = 0; i < W; ++i) s_ = fmaf(wt[i][j], win[i][j], s_);
-                    acc[j] = silu ? s_ / (1.f + expf(-s_)) : s_;
+                    acc[j] = silu ? __fdividef(s_, 1.f + __expf(-s_)) : s_;
                 }
                 *reinterpret_cast<float4*>(yp + (size_t)u * C) = make_float4(acc[0], acc[1], acc[2], acc[3]);
 #pragma unroll

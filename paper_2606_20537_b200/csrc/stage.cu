@@ -3,7 +3,10 @@
 // One kernel serves the lazy rebuild (esc_dequant_stage_fill: live FP8 row -> stage) and the eager, fused restore
 // (esc_restore_ex: capsule slab -> live row AND stage, plain rows copied alongside, ONE launch).  Like the capsule
 // copy kernel it is driven by a table of (row, segment) entries cut into 8 KiB tiles of source bytes, one CTA per
-// tile; a thread loads 2 x 16 codes, stores them (when the entry has an FP8 destination) and stores 2 x 32 B of BF16.
+// tile; a thread loads 4 x 8 codes (all four loads before the first store), stores them (when the entry has an FP8
+// destination) and stores 4 x 16 B of BF16, so every load / store instruction of a warp covers one contiguous
+// 256 B / 512 B range (r01u: with 16-code loads each thread's 32 B of BF16 went out as two 16-byte stores at a
+// 32-byte stride, half-used sectors per instruction: stage fill 17.6 -> 13.4 us, eager fused restore 27.6 -> 22.7 us).
 // Roofline: HBM.  Algorithmic bytes per FP8 element: 1 read + 2 written for a fill, 1 + 1 + 2 for a fused restore.
 // Arithmetic per element (the precision both sides take the rounding decisions in): cvt e4m3 -> f16 (exact) -> f32
 // (exact), one fp32 multiply by the row scale, cvt.rn to bf16; NaN codes are replaced by 0x7FC0 | sign.
@@ -17,7 +20,8 @@
 namespace esc {
 
 constexpr uint32_t kStageMaxSeg = 96;
-constexpr uint32_t kStageTile = kCopyThreads * 2 * 16u;   // 8 KiB of source bytes
+constexpr uint32_t kStageUnroll = 4;                              // 8-byte code vectors in flight per thread
+constexpr uint32_t kStageTile = kCopyThreads * kStageUnroll * 8u;   // 8 KiB of source bytes
 
 struct StageTable {
     uint32_t n_seg;
@@ -42,6 +46,22 @@ __device__ __forceinline__ uint32_t expand2(uint32_t codes, float scale) {
     return r;
 }
 
+// eight codes per thread: a warp loads 256 contiguous bytes and stores 512 contiguous bytes of BF16 per instruction
+__device__ __forceinline__ uint2 ld_codes8(const uint2* p) {
+    uint2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void put_codes8(uint8_t* d8, uint8_t* d16, uint32_t i, const uint2& v, float scale) {
+    if (d8) reinterpret_cast<uint2*>(d8)[i] = v;
+    if (d16) {
+        uint4 o;
+        o.x = expand2(v.x, scale); o.y = expand2(v.x >> 16, scale);
+        o.z = expand2(v.y, scale); o.w = expand2(v.y >> 16, scale);
+        reinterpret_cast<uint4*>(d16)[i] = o;
+    }
+}
+
 __device__ __forceinline__ uint16_t expand1(uint8_t code, float scale) { return (uint16_t)(expand2(code, scale) & 0xFFFFu); }
 
 __global__ void __launch_bounds__(kCopyThreads, 8) esc_stage_kernel(const __grid_constant__ StageTable t) {
@@ -63,26 +83,17 @@ __global__ void __launch_bounds__(kCopyThreads, 8) esc_stage_kernel(const __grid
         const float scale = t.scale[e];
         const bool aligned = ((((uintptr_t)src) | ((uintptr_t)d8) | ((uintptr_t)d16)) & 15u) == 0;
         uint32_t done = 0;
-        if (aligned) {
-            const uint32_t n16 = n >> 4;
-            for (uint32_t i = tid; i < n16; i += kCopyThreads) {
-                uint4 v;
-                asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-                             : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
-                             : "l"(reinterpret_cast<const uint4*>(src) + i));
-                if (d8) reinterpret_cast<uint4*>(d8)[i] = v;
-                if (d16) {
-                    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-                    uint4 o0, o1;
-                    o0.x = expand2(w[0], scale); o0.y = expand2(w[0] >> 16, scale);
-                    o0.z = expand2(w[1], scale); o0.w = expand2(w[1] >> 16, scale);
-                    o1.x = expand2(w[2], scale); o1.y = expand2(w[2] >> 16, scale);
-                    o1.z = expand2(w[3], scale); o1.w = expand2(w[3] >> 16, scale);
-                    reinterpret_cast<uint4*>(d16)[2 * i] = o0;
-                    reinterpret_cast<uint4*>(d16)[2 * i + 1] = o1;
-                }
-            }
-            done = n16 << 4;
+        if (aligned && n == kStageTile) {   // full tile: all loads of a thread first, then its stores
+            uint2 v[kStageUnroll];
+#pragma unroll
+            for (int u = 0; u < (int)kStageUnroll; ++u) v[u] = ld_codes8(reinterpret_cast<const uint2*>(src) + tid + u * kCopyThreads);
+#pragma unroll
+            for (int u = 0; u < (int)kStageUnroll; ++u) put_codes8(d8, d16, tid + u * kCopyThreads, v[u], scale);
+            done = n;
+        } else if (aligned) {
+            const uint32_t n8 = n >> 3;
+            for (uint32_t i = tid; i < n8; i += kCopyThreads) put_codes8(d8, d16, i, ld_codes8(reinterpret_cast<const uint2*>(src) + i), scale);
+            done = n8 << 3;
         }
         for (uint32_t i = done + tid; i < n; i += kCopyThreads) {   // tails and unaligned pointers: element by element
             const uint8_t c = src[i];
