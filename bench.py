@@ -245,7 +245,7 @@ def run_esc(args):
         caps[j] = esc.snapshot(sess.set, P_STEP, CHUNK, slabs[j], stream=stream)
         g.set_capsule(caps[(j + N_CAPSULES // 2) % N_CAPSULES], stream)   # written 10 steps ago: not in L2
         g.launch(stream)
-        launches[0] += 2 + N_LINEAR
+        launches[0] += 3 + N_LINEAR     # snapshot copy, table store, restore copy, one scan per linear layer
 
     def timed(fn, n, with_flush=True):
         pairs = []
@@ -299,6 +299,7 @@ def run_esc(args):
         ev_in = [torch.cuda.Event() for _ in range(n)]
         ev_cmp = [torch.cuda.Event() for _ in range(n)]
         ev_out = [torch.cuda.Event() for _ in range(n)]
+        h0 = time.perf_counter()
         t0.record(stream)
         s_in.wait_event(t0)
         for i in range(n):
@@ -321,8 +322,10 @@ def run_esc(args):
         if n >= 2:
             stream.wait_event(ev_out[n - 2])
         t1.record(stream)
+        host_ms[0] = (time.perf_counter() - h0) * 1e3 / n     # host time to enqueue one step (before the final sync)
         torch.cuda.synchronize()
         return t0.elapsed_time(t1) / n
+    host_ms = [0.0]
     run_pipelined(max(args.warmup, 3))
     ms_e2e = run_pipelined(args.steps)
     graph_b.destroy()
@@ -388,7 +391,7 @@ def run_esc(args):
                    "value_definition": "4 x capsule bytes (snapshot r+w, restore r+w) / step time, all ranks"},
         "clocks": clocks, "gpu_launches": n_launch, "wall_ms_timed_region": wall_ms,
         "e2e": {"value": e2e_value, "unit": "GB/s", "h2d_bytes_per_step": inputs.h2d_bytes(),
-                "d2h_bytes_per_step": inputs.d2h_bytes(), "ms_per_step": ms_e2e,
+                "d2h_bytes_per_step": inputs.d2h_bytes(), "ms_per_step": ms_e2e, "host_enqueue_ms_per_step": host_ms[0],
                 "mode": "K steps back to back, double-buffered: H2D of step i+1 and D2H of step i-1 overlap step i "
                         "(separate streams); every step uploads its inputs from pinned memory and downloads its outputs",
                 "serial_ms_per_step": ms_e2e_serial, "serial_value": aggregate_value(moved, ms_e2e_serial, world),

@@ -23,7 +23,7 @@
  *   - Ownership: the library NEVER allocates or frees tensor memory.  Live buffers and
  *     capsule storage slabs are caller-owned device memory (the Python binding uses
  *     torch tensors).  The library owns only its small host structs and, per esc_graph,
- *     one device-resident descriptor table (a few KiB) + its pinned host mirror.
+ *     one device-resident descriptor table (a few KiB), rewritten by a one-CTA kernel.
  *   - Streams: every verb only ENQUEUES work on the caller's cudaStream_t (passed as
  *     void*; NULL = legacy default stream) and returns without a host sync.  Everything
  *     the host can detect (bad arguments, layout / digest mismatch, unaligned boundary,
@@ -311,7 +311,8 @@ typedef struct esc_scan_args {
 int esc_graph_capture(esc_ctx* ctx, esc_bufset* live, uint64_t max_boundary,
                       const esc_scan_args* layers, uint32_t n_layers, void* stream, esc_graph** out_graph);
 /* Bind the capsule the next launches restore from: host rebuilds the table and enqueues one
- * small async H2D copy on `stream`.  Same layout / capacity checks as esc_restore. */
+ * small kernel on `stream` that stores it to the graph's device-resident copy (the table travels as a
+ * kernel parameter: no copy engine, no host-side wait; the call may be repeated at any rate).  Same layout / capacity checks as esc_restore. */
 int esc_graph_set_capsule(esc_graph* graph, const esc_bufset* capsule, void* stream);
 /* One cudaGraphLaunch on `stream`.  ESC_ERR_INVALID if the plan has a restore node and no
  * capsule is bound. */

@@ -117,6 +117,8 @@ int launch_fork(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* c
 // table-in-global-memory variant used inside captured graphs
 void build_copy_table(CopyTable* t, const uint8_t* const* src, uint8_t* const* dst, const uint64_t* bytes, uint32_t n);
 int launch_copy_indirect(const esc_ctx* ctx, const CopyTable* table_dev, uint32_t grid_blocks, cudaStream_t stream);
+// stores t (passed by value as a kernel parameter) to the device-resident table on `stream`
+int launch_table_store(const CopyTable& t, CopyTable* table_dev, cudaStream_t stream);
 
 // staged copy / FP8 -> BF16 expansion (stage.cu): entry i copies bytes[i] from src to dst8 (if not NULL) and writes
 // their BF16 expansion to dst16 (if not NULL)

@@ -13,9 +13,7 @@ struct esc_graph {
     esc_bufset* live;             // NULL: cold plan (no restore node)
     cudaGraph_t graph;
     cudaGraphExec_t exec;
-    esc::CopyTable* table_dev;    // device-resident "current capsule" table
-    esc::CopyTable* table_host;   // pinned mirror
-    cudaEvent_t table_copied;     // guards reuse of the pinned mirror
+    esc::CopyTable* table_dev;    // device-resident "current capsule" table (rewritten by a one-CTA kernel: launch_table_store)
     bool bound;
     uint64_t bound_boundary;
 };
@@ -35,8 +33,6 @@ static void graph_free(esc_graph* g) {
     if (g->exec) cudaGraphExecDestroy(g->exec);
     if (g->graph) cudaGraphDestroy(g->graph);
     if (g->table_dev) cudaFree(g->table_dev);
-    if (g->table_host) cudaFreeHost(g->table_host);
-    if (g->table_copied) cudaEventDestroy(g->table_copied);
     delete g;
 }
 
@@ -81,8 +77,6 @@ int esc_graph_capture(esc_ctx* ctx, esc_bufset* live, uint64_t max_boundary, con
     cudaError_t e = cudaSuccess;
     if (live) {
         e = cudaMalloc((void**)&g->table_dev, sizeof(CopyTable));
-        if (e == cudaSuccess) e = cudaMallocHost((void**)&g->table_host, sizeof(CopyTable));
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->table_copied, cudaEventDisableTiming);
         if (e == cudaSuccess) e = cudaMemset(g->table_dev, 0, sizeof(CopyTable));  // n_tiles = 0: a no-op until bound
         if (e != cudaSuccess) {
             graph_free(g);
@@ -133,11 +127,10 @@ int esc_graph_set_capsule(esc_graph* graph, const esc_bufset* capsule, void* str
         dst[i] = segs[i].live;
         bytes[i] = segs[i].bytes;
     }
-    ESC_CUDA(cudaEventSynchronize(graph->table_copied));  // previous upload has left the pinned mirror
-    build_copy_table(graph->table_host, src.data(), dst.data(), bytes.data(), (uint32_t)segs.size());
-    ESC_CUDA(cudaMemcpyAsync(graph->table_dev, graph->table_host, sizeof(CopyTable), cudaMemcpyHostToDevice,
-                             (cudaStream_t)stream));
-    ESC_CUDA(cudaEventRecord(graph->table_copied, (cudaStream_t)stream));
+    CopyTable t;
+    build_copy_table(&t, src.data(), dst.data(), bytes.data(), (uint32_t)segs.size());
+    rc = launch_table_store(t, graph->table_dev, (cudaStream_t)stream);
+    if (rc != ESC_OK) return rc;
     graph->bound = true;
     graph->bound_boundary = capsule->position;
     return ESC_OK;
