@@ -39,7 +39,7 @@ def parse_args():
     ap.add_argument("--impl", default="esc", choices=["esc", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the scan / warm-vs-cold / cpu_baseline extras")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--profile", default=None, choices=["scan", "restore", "suffix", "gdn"],
+    ap.add_argument("--profile", default=None, choices=["scan", "restore", "suffix", "gdn", "conv", "stage"],
                     help="ncu driver: launch only the cold 16448-token scan (x3), only the 66 MiB restore (x5) or only the 18 "
                          "64-token suffix scans (x2); no JSON line")
     return ap.parse_args()
@@ -637,6 +637,31 @@ def run_profile(args):
         key = esc.shape_key_make(1, 16, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
         for _ in range(3):
             esc.gdn_scan(ctx, key, *full.dev[0], beta, None, sess.states[0], full.out[0], T, T, stream=stream)
+    elif args.profile == "conv":
+        T, Cc, Wc = 16384 + SUFFIX, 3 * workload.H * 128, 4
+        cx = torch.randn((1, T, Cc), device="cuda:0").to(torch.bfloat16)
+        cw = torch.randn((Cc, Wc), device="cuda:0")
+        cst = torch.zeros((1, Cc, Wc - 1), device="cuda:0")
+        cy = torch.empty((1, T, Cc), dtype=torch.float32, device="cuda:0")
+        for _ in range(3):
+            esc.causal_conv(ctx, cx, cw, cst, cst, cy, 1, T, T, Cc, Wc, esc.CONV_SILU, stream=stream)
+    elif args.profile == "stage":
+        from paper_2606_20537_b200 import synth
+        specs8 = synth.hybrid_layout(P_STEP + SUFFIX, kv_elem_bytes=1)
+        bufs8 = [torch.randint(0, 256, (sp.capacity_bytes,), dtype=torch.uint8, device="cuda:0") for sp in specs8]
+        live8 = esc.bufset_create(ctx, [(sp.name, b_, sp.capacity_bytes, sp.fixed_bytes, sp.bytes_per_token, sp.n_seg, sp.seg_stride)
+                                        for sp, b_ in zip(specs8, bufs8)])
+        kv_rows = [i for i, sp in enumerate(specs8) if sp.bytes_per_token]
+        stages8 = [torch.empty(specs8[i].capacity_bytes, dtype=torch.bfloat16, device="cuda:0") for i in kv_rows]
+        for i, st in zip(kv_rows, stages8):
+            live8.attach_dequant_stage(i, st, scale=0.25)
+        live8.set_position(P_STEP)
+        slabs8 = [torch.empty(live8.capsule_bytes(P_STEP)[0], dtype=torch.uint8, device="cuda:0") for _ in range(4)]
+        caps8 = [esc.snapshot(live8, P_STEP, CHUNK, s8, stream=stream) for s8 in slabs8]
+        for c8 in caps8:                                   # esc_stage_kernel launches 1, 3, 5, 7: eager fused restores
+            esc.restore_ex(live8, c8, flags=esc.RESTORE_DEQUANT_EAGER, stream=stream)
+            esc.restore(live8, c8, stream=stream)          # resets the stages' valid ends
+            live8.stage_fill(esc.ALL_ROWS, P_STEP, stream=stream)   # launches 2, 4, 6, 8: lazy fills of all 12 KV rows
     elif args.profile == "suffix":
         sess = workload.HybridSession(ctx, P_STEP + SUFFIX, seed=0)
         inputs = workload.SuffixInputs(N_LINEAR, SUFFIX, seed=0)
