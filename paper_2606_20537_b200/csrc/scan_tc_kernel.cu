@@ -41,6 +41,7 @@
 //   warps 8-11     score warps (one per TMEM lane quadrant): P slice (TMEM) -> A slice -> all CTAs
 //   warps 12-15    state warps: U (TMEM) -> carry S in fp32 registers -> [S_hi | S_lo] operand
 //   warps 16-19    epilogue warps: O1, O2 (TMEM) -> o (global)
+//   warps 22-25    (cluster-free variant only) second set of score warps: the upper half of the key columns
 //
 // Bit-identity: the carry is a pure function of (S_prev bits, chunk inputs); there
 // is no T-dependent tiling, no atomics, no split-K; every accumulator is produced by ONE issuer thread
@@ -60,6 +61,17 @@ typedef __nv_bfloat16 bf16;
 
 constexpr int kTcWarps = 22;
 constexpr int kTcThreads = kTcWarps * 32;
+// The cluster-free (short-call) variant runs a second set of four score warps (warps 22-25): each set takes half of the C key
+// columns of every row quadrant, which halves the longest score warp's work on the one-chunk critical path
+// (r01u, 18-layer suffix graph: 4.78 -> 4.55 us per layer; same elements by the same expressions: bit-identical).
+#ifndef ESC_TC_SW
+#define ESC_TC_SW 2
+#endif
+template <int CS> struct TcScore {
+    static constexpr int sets = CS == 1 ? ESC_TC_SW : 1;
+    static constexpr int threads = (kTcWarps + 4 * (sets - 1)) * 32;
+};
+constexpr int kTcThreadsMax = (kTcWarps + 4) * 32;
 constexpr int kTcDVT = 16;        // d_v columns per CTA
 constexpr int kTcNM = 2 * kTcDVT; // columns of a merged hi|lo operand
 constexpr int kGateBatch = 256;   // tokens per gate-warp batch
@@ -185,7 +197,7 @@ __device__ __forceinline__ void tmem_ld_slice(uint32_t addr, uint32_t* r) {
 }
 
 template <int DK, int C, int CS, typename OutT>
-__global__ void __launch_bounds__(kTcThreads, 1)
+__global__ void __launch_bounds__(kTcThreadsMax, 1)
 esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tk,
                    const __grid_constant__ CUtensorMap tv, const float* __restrict__ g, const float* state_in,
                    float* state_out, OutT* __restrict__ o, uint32_t H, uint32_t DV, uint64_t T, uint64_t t_stride) {
@@ -193,6 +205,8 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     constexpr TcBars BI = tc_bars<DK, C, CS>();
     constexpr int NS = L::NS, NB = L::NB, NSB = L::NSB, CPB = L::CPB;
     constexpr int NA = C / CS;                      // keys per score slice = Q / K rows this CTA loads
+    constexpr int SW = TcScore<CS>::sets;           // score-warp sets (each takes NA / SW of the slice's key columns)
+    constexpr int NAW = NA / SW;
     constexpr uint16_t kAll = (uint16_t)((1u << CS) - 1);
     constexpr uint32_t SBO_V = (C / 8) * 128, SBO_S = (DK / 8) * 128;
     static_assert(NA == 8 || NA == 16 || NA == 32 || NA == 64, "slice width");
@@ -263,15 +277,15 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     if (warp == 0 && lane == 0) {
         for (int i = 0; i < NS; ++i) { mbar_init(&bars[BI.full + i], 1); mbar_init(&bars[BI.empty + i], 3 * CS); }
         for (int i = 0; i < NB; ++i) {
-            mbar_init(&bars[BI.p_full + i], 1); mbar_init(&bars[BI.p_empty + i], 4);
-            mbar_init(&bars[BI.a_full + i], 4); mbar_init(&bars[BI.a_empty + i], CS);
+            mbar_init(&bars[BI.p_full + i], 1); mbar_init(&bars[BI.p_empty + i], 4 * SW);
+            mbar_init(&bars[BI.a_full + i], 4 * SW); mbar_init(&bars[BI.a_empty + i], CS);
             mbar_init(&bars[BI.vt_full + i], 4); mbar_init(&bars[BI.vt_empty + i], 2);
         }
         for (int i = 0; i < NSB; ++i) { mbar_init(&bars[BI.s_full + i], 4); mbar_init(&bars[BI.s_empty + i], 1); }
         for (int i = 0; i < 2; ++i) {
             mbar_init(&bars[BI.o1_full + i], 1); mbar_init(&bars[BI.o2_full + i], 1); mbar_init(&bars[BI.o_empty + i], 4);
             mbar_init(&bars[BI.u_full + i], 1); mbar_init(&bars[BI.u_empty + i], 4);
-            mbar_init(&bars[BI.g_full + i], 1); mbar_init(&bars[BI.g_empty + i], 16);
+            mbar_init(&bars[BI.g_full + i], 1); mbar_init(&bars[BI.g_empty + i], 16 + 4 * (SW - 1));
         }
         fence_mbar_init();
         tma_prefetch_desc(&tq); tma_prefetch_desc(&tk); tma_prefetch_desc(&tv);
@@ -515,7 +529,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             }
         }
     }
-    else if (warp >= 8 && warp < 12) {
+    else if ((warp >= 8 && warp < 12) || warp >= kTcWarps) {
         // ================= score warps: A[:, slice] = P[:, slice] ⊙ 2^(b_i - b_j) (causal) -> every CTA of the cluster =================
         // One warp per TMEM lane quadrant.  A quadrant holds 16 rows of an M = 64 tile (row r in lane 32(r/16) + r%16) or 32
         // rows of an M = 128 tile (row r in lane r): NG 16-row groups per warp.  A group whose rows all precede the slice's
@@ -524,18 +538,19 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
         constexpr uint32_t kSlice = (NA / 8) * L::a_lbo;           // bytes of one CTA's slice
         constexpr uint32_t tx = (CS - 1) * kSlice;                  // what the peers push into this CTA's A buffer per chunk
         auto rows_base = [&](int qq, int gi) { return (C == 64) ? 16 * qq : 32 * qq + 16 * gi; };
-        bool act[NG];
+        const uint32_t kw0 = key0 + (warp >= kTcWarps ? NAW : 0);   // first key column of this warp
+        bool act[NG];   // (a CTA on its own writes all of A itself: masked groups as zeros)
 #pragma unroll
-        for (int gi = 0; gi < NG; ++gi) act[gi] = (uint32_t)rows_base(q, gi) + 15 >= key0;
+        for (int gi = 0; gi < NG; ++gi) act[gi] = CS == 1 || (uint32_t)rows_base(q, gi) + 15 >= key0;
         for (uint32_t c = 0; c < n_chunks; ++c) {
             const uint32_t pb = c % NB, bt = c / CPB, gslot = bt & 1;
             mbar_wait(&bars[BI.g_full + gslot], (bt >> 1) & 1);
             const float* b2 = gate + gslot * 2 * kGateBatch + (c % CPB) * C;
             if (q == 3 && lane == 0) TC_TRACE(5, c);
             // every b_j is read before the first A store (the stores may alias b2 as far as the compiler can tell)
-            float2 bj[NA / 8];
+            float2 bj[NAW / 8];
 #pragma unroll
-            for (int jb = 0; jb < NA / 8; ++jb) bj[jb] = *reinterpret_cast<const float2*>(b2 + key0 + jb * 8 + 2 * (lane & 3));
+            for (int jb = 0; jb < NAW / 8; ++jb) bj[jb] = *reinterpret_cast<const float2*>(b2 + kw0 + jb * 8 + 2 * (lane & 3));
             float bi[NG][2];
 #pragma unroll
             for (int gi = 0; gi < NG; ++gi) {
@@ -545,10 +560,11 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             mbar_wait(&bars[BI.a_empty + pb], ((c / NB) & 1) ^ 1);   // all CS CTAs are done reading A buffer pb (chunk c - NB)
             mbar_wait(&bars[BI.p_full + pb], (c / NB) & 1);
             tc_fence_after_sync();
-            uint32_t r[NG][NA / 2];
+            uint32_t r[NG][NAW / 2];
 #pragma unroll
             for (int gi = 0; gi < NG; ++gi)
-                if (act[gi]) tmem_ld_slice<NA>(tmem_addr(tb, (C == 64) ? 32 * q : 32 * q + 16 * gi, L::tm_p + pb * L::p_cols), r[gi]);
+                if (act[gi])
+                    tmem_ld_slice<NAW>(tmem_addr(tb, (C == 64) ? 32 * q : 32 * q + 16 * gi, L::tm_p + pb * L::p_cols + (kw0 - key0)), r[gi]);
             tmem_ld_wait();
             tc_fence_before_sync();
             __syncwarp();
@@ -558,10 +574,10 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             for (int gi = 0; gi < NG; ++gi) {
                 if (act[gi]) {
                     const int ra = rows_base(q, gi) + (lane >> 2), rb = ra + 8;
-                    uint32_t hi_a[NA / 8], lo_a[NA / 8], hi_c[NA / 8], lo_c[NA / 8];
+                    uint32_t hi_a[NAW / 8], lo_a[NAW / 8], hi_c[NAW / 8], lo_c[NAW / 8];
 #pragma unroll
-                    for (int jb = 0; jb < NA / 8; ++jb) {
-                        const int j0 = (int)key0 + jb * 8 + 2 * (lane & 3);
+                    for (int jb = 0; jb < NAW / 8; ++jb) {
+                        const int j0 = (int)kw0 + jb * 8 + 2 * (lane & 3);
                         float a0 = __uint_as_float(r[gi][4 * jb + 0]) * ex2(bi[gi][0] - bj[jb].x);
                         float a1 = __uint_as_float(r[gi][4 * jb + 1]) * ex2(bi[gi][0] - bj[jb].y);
                         float c0 = __uint_as_float(r[gi][4 * jb + 2]) * ex2(bi[gi][1] - bj[jb].x);
@@ -575,8 +591,8 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
                     }
                     uint8_t* arow = ab + (ra >> 3) * 128 + (ra & 7) * 16 + (lane & 3) * 4;
 #pragma unroll
-                    for (int jb = 0; jb < NA / 8; ++jb) {
-                        uint8_t* pa = arow + (key0 / 8 + jb) * L::a_lbo;
+                    for (int jb = 0; jb < NAW / 8; ++jb) {
+                        uint8_t* pa = arow + (kw0 / 8 + jb) * L::a_lbo;
                         *reinterpret_cast<uint32_t*>(pa) = hi_a[jb];
                         *reinterpret_cast<uint32_t*>(pa + L::a_term) = lo_a[jb];
                         *reinterpret_cast<uint32_t*>(pa + 128) = hi_c[jb];              // row + 8
@@ -589,7 +605,7 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             // the slice of this CTA (all rows, both terms: NA/8 consecutive 8-key groups) is one contiguous range of the A
             // buffer: once the four score warps have written it, one lane per peer pushes it into the same place of that
             // peer's buffer pb; the copy completes (tx bytes) on the peer's a_full barrier
-            asm volatile("bar.sync 1, 128;" ::: "memory");
+            if constexpr (CS > 1) asm volatile("bar.sync 1, 128;" ::: "memory");   // (on its own a CTA has nobody to push to)
             if constexpr (CS > 1) if (q == 0 && lane + 1 < CS) {
                 const uint32_t d = (uint32_t)lane + ((uint32_t)lane >= rank ? 1u : 0u);
                 const uint32_t off = L::a_off + pb * L::a_bytes + (key0 / 8) * L::a_lbo;
@@ -766,7 +782,7 @@ static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const v
     if (rc != ESC_OK) return rc;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(s.dv / kTcDVT, s.B * s.H);   // d_v / 16 CTAs per (b, h), in clusters of CS
-    cfg.blockDim = dim3(kTcThreads);
+    cfg.blockDim = dim3(TcScore<CS>::threads);
     cfg.dynamicSmemBytes = L::total;
     cfg.stream = stream;
     cudaLaunchAttribute attr[2];
