@@ -245,10 +245,15 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
     // TMA producer steps (warp 0, lane 0)
     auto tma_prefetch_chunk = [&](uint32_t c) {   // pull this CTA's share of chunk c into L2
         const int t0 = (int)(c * C);
+        if constexpr (CS == 1) {
+            tma_prefetch_5d(&tq, 0, t0, 0, (int)h, (int)b);
+            tma_prefetch_5d(&tk, 0, t0, 0, (int)h, (int)b);
+        } else {
 #pragma unroll
-        for (int hh = 0; hh < L::NH; ++hh) {
-            tma_prefetch_4d(&tq, hh * 64, (int)h, t0 + (int)key0, (int)b);
-            tma_prefetch_4d(&tk, hh * 64, (int)h, t0 + (int)key0, (int)b);
+            for (int hh = 0; hh < L::NH; ++hh) {
+                tma_prefetch_4d(&tq, hh * 64, (int)h, t0 + (int)key0, (int)b);
+                tma_prefetch_4d(&tk, hh * 64, (int)h, t0 + (int)key0, (int)b);
+            }
         }
         tma_prefetch_4d(&tv, (int)dv0, (int)h, t0, (int)b);
     };
@@ -258,16 +263,19 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
         uint64_t* full = &bars[BI.full + s];
         mbar_arrive_expect_tx(full, L::stage_bytes);   // Q and K arrive in CS row slices, one from each CTA
         const int t0 = (int)(c * C);
+        if constexpr (CS > 1) {
 #pragma unroll
-        for (int hh = 0; hh < L::NH; ++hh) {
-            if constexpr (CS > 1) {
+            for (int hh = 0; hh < L::NH; ++hh) {
                 tma_load_4d_mc(st + hh * L::half_bytes + key0 * 128, &tq, full, hh * 64, (int)h, t0 + (int)key0, (int)b, kAll);
                 tma_load_4d_mc(st + L::q_bytes + hh * L::half_bytes + key0 * 128, &tk, full, hh * 64, (int)h, t0 + (int)key0, (int)b,
                                kAll);
-            } else {
-                tma_load_4d(st + hh * L::half_bytes, &tq, full, hh * 64, (int)h, t0, (int)b);
-                tma_load_4d(st + L::q_bytes + hh * L::half_bytes, &tk, full, hh * 64, (int)h, t0, (int)b);
             }
+        } else {
+            // on its own a CTA takes a whole tile per instruction: the map has the 64-column halves as its third dimension
+            // (d % 64, t, d / 64, h, b), so a box of (64, C, NH) lands as [half][token][64] — the two half tiles back to back
+            // (r01u trace: the producer needs ~200 cycles per TMA instruction, and a one-chunk call waits for all of them)
+            tma_load_5d(st, &tq, full, 0, t0, 0, (int)h, (int)b);
+            tma_load_5d(st + L::q_bytes, &tk, full, 0, t0, 0, (int)h, (int)b);
         }
         tma_load_4d(st + 2 * L::q_bytes, &tv, full, (int)dv0, (int)h, t0, (int)b);
         TC_TRACE(0, c);
@@ -761,6 +769,23 @@ static int make_tmap(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, u
     return r == CUDA_SUCCESS ? ESC_OK : ESC_ERR_CUDA;
 }
 
+// whole Q / K tiles for the cluster-free variant: dimensions (d % 64, t, d / 64, h, b), box (64, box_t, D / 64, 1, 1)
+static int make_tmap_halves(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, uint64_t T, uint64_t t_stride, uint32_t B,
+                            uint32_t box_t) {
+    TmapEncodeFn enc = tmap_encode_fn();
+    if (!enc) return ESC_ERR_CUDA;
+    const uint32_t nh = D / 64;
+    cuuint64_t dims[5] = {64, T ? T : 1, nh, H, B};
+    cuuint64_t strides[4] = {(cuuint64_t)H * D * 2, 128, (cuuint64_t)D * 2, (cuuint64_t)t_stride * H * D * 2};
+    cuuint32_t box[5] = {64, box_t, nh, 1, 1};
+    cuuint32_t es[5] = {1, 1, 1, 1, 1};
+    if (B == 1) strides[3] = strides[0] * dims[1];   // unused dimension: any valid multiple of 16
+    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void*>(base), dims, strides, box, es,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? ESC_OK : ESC_ERR_CUDA;
+}
+
 template <int DK, int C, int CS, typename OutT>
 static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                        float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
@@ -776,8 +801,14 @@ static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const v
     const void* kk = T ? k : (const void*)state_out;
     const void* vv = T ? v : (const void*)state_out;
     // Q / K: each CTA of the cluster loads (and multicasts) C / CS rows of a chunk; V: the CTA's own 16 columns
-    int rc = make_tmap(&tq, qq, DK, s.H, T, t_stride ? t_stride : 1, s.B, 64, C / CS, CU_TENSOR_MAP_SWIZZLE_128B);
-    if (rc == ESC_OK) rc = make_tmap(&tk, kk, DK, s.H, T, t_stride ? t_stride : 1, s.B, 64, C / CS, CU_TENSOR_MAP_SWIZZLE_128B);
+    int rc;
+    if (CS == 1) {
+        rc = make_tmap_halves(&tq, qq, DK, s.H, T, t_stride ? t_stride : 1, s.B, C);
+        if (rc == ESC_OK) rc = make_tmap_halves(&tk, kk, DK, s.H, T, t_stride ? t_stride : 1, s.B, C);
+    } else {
+        rc = make_tmap(&tq, qq, DK, s.H, T, t_stride ? t_stride : 1, s.B, 64, C / CS, CU_TENSOR_MAP_SWIZZLE_128B);
+        if (rc == ESC_OK) rc = make_tmap(&tk, kk, DK, s.H, T, t_stride ? t_stride : 1, s.B, 64, C / CS, CU_TENSOR_MAP_SWIZZLE_128B);
+    }
     if (rc == ESC_OK) rc = make_tmap(&tv, vv, s.dv, s.H, T, t_stride ? t_stride : 1, s.B, kTcDVT, C, CU_TENSOR_MAP_SWIZZLE_32B);
     if (rc != ESC_OK) return rc;
     cudaLaunchConfig_t cfg = {};
