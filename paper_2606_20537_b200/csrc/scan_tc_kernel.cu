@@ -41,7 +41,7 @@
 //   warps 8-11     score warps (one per TMEM lane quadrant): P slice (TMEM) -> A slice -> all CTAs
 //   warps 12-15    state warps: U (TMEM) -> carry S in fp32 registers -> [S_hi | S_lo] operand
 //   warps 16-19    epilogue warps: O1, O2 (TMEM) -> o (global)
-//   warps 22-25    (cluster-free variant only) second set of score warps: the upper half of the key columns
+//   warps 22-25    second set of score warps: the upper half of the slice's key columns
 //
 // Bit-identity: the carry is a pure function of (S_prev bits, chunk inputs); there
 // is no T-dependent tiling, no atomics, no split-K; every accumulator is produced by ONE issuer thread
@@ -61,14 +61,19 @@ typedef __nv_bfloat16 bf16;
 
 constexpr int kTcWarps = 22;
 constexpr int kTcThreads = kTcWarps * 32;
-// The cluster-free (short-call) variant runs a second set of four score warps (warps 22-25): each set takes half of the C key
+// Both variants run a second set of four score warps (warps 22-25; first for the cluster-free short-call variant): each set takes half of the C key
 // columns of every row quadrant, which halves the longest score warp's work on the one-chunk critical path
 // (r01u, 18-layer suffix graph: 4.78 -> 4.55 us per layer; same elements by the same expressions: bit-identical).
 #ifndef ESC_TC_SW
 #define ESC_TC_SW 2
 #endif
+// The cluster variant runs the second set too (each set 8 of the slice's 16 key columns): 211 -> 207 us at 16 448 tokens,
+// -2 % across the config-4 sweep, -6 % at T = 2048 (r01u).
+#ifndef ESC_TC_SW_LONG
+#define ESC_TC_SW_LONG 2
+#endif
 template <int CS> struct TcScore {
-    static constexpr int sets = CS == 1 ? ESC_TC_SW : 1;
+    static constexpr int sets = CS == 1 ? ESC_TC_SW : ESC_TC_SW_LONG;
     static constexpr int threads = (kTcWarps + 4 * (sets - 1)) * 32;
 };
 constexpr int kTcThreadsMax = (kTcWarps + 4) * 32;
@@ -613,15 +618,18 @@ esc_scan_tc_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant
             // the slice of this CTA (all rows, both terms: NA/8 consecutive 8-key groups) is one contiguous range of the A
             // buffer: once the four score warps have written it, one lane per peer pushes it into the same place of that
             // peer's buffer pb; the copy completes (tx bytes) on the peer's a_full barrier
-            if constexpr (CS > 1) asm volatile("bar.sync 1, 128;" ::: "memory");   // (on its own a CTA has nobody to push to)
-            if constexpr (CS > 1) if (q == 0 && lane + 1 < CS) {
+            if constexpr (CS > 1) {   // (on its own a CTA has nobody to push to)
+                if constexpr (SW == 1) asm volatile("bar.sync 1, 128;" ::: "memory");
+                else asm volatile("bar.sync 1, 256;" ::: "memory");
+            }
+            if constexpr (CS > 1) if (q == 0 && warp < kTcWarps && lane + 1 < CS) {
                 const uint32_t d = (uint32_t)lane + ((uint32_t)lane >= rank ? 1u : 0u);
                 const uint32_t off = L::a_off + pb * L::a_bytes + (key0 / 8) * L::a_lbo;
                 bulk_copy_to_cluster(mapa(sm_a + off, d), sm_a + off, kSlice, mapa(smem_u32(&bars[BI.a_full + pb]), d));
             }
             if (q == 3 && lane == 0) TC_TRACE(6, c);
             if (lane == 0) {
-                if (CS > 1 && q == 3) mbar_arrive_expect_tx(&bars[BI.a_full + pb], tx);   // quadrant 3 holds the last rows: always active
+                if (CS > 1 && q == 3 && warp < kTcWarps) mbar_arrive_expect_tx(&bars[BI.a_full + pb], tx);   // quadrant 3 holds the last rows: always active
                 else mbar_arrive(&bars[BI.a_full + pb]);
                 if ((c % CPB) == (uint32_t)CPB - 1 || c + 1 == n_chunks) mbar_arrive(&bars[BI.g_empty + gslot]);
             }
