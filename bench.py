@@ -372,7 +372,7 @@ def run_esc(args):
     roof_sfx = {"kernel": "esc_scan_tc_kernel<128,64,1,float> (B1 H16 d128, T=64 suffix: one chunk per (b,h); 18 launches per step)",
                 "bound": "hbm", "achieved": sfx_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": sfx_gbs / pk["hbm_gbs"],
                 "peak_source": pk["source"], "traffic": 1.89e6, "us_per_launch": sfx_us, "alg_bytes_per_launch": sfx_alg,
-                "traffic_note": "ncu r01s (profiles/r01s_suffix_scan_ncu_full.txt): dram read 1.89 MB, write 0 in the kernel's window "
+                "traffic_note": "ncu r01u (profiles/r01u_suffix_scan_ncu_full.txt): dram read 1.89 MB, write 0 in the kernel's window "
                                 "(state and outputs still dirty in L2 at kernel end)",
                 "share_of_step": ms_suffix / ms_step,
                 "note": "latency-bound by construction: 3.4 MB per launch is 0.5 us of HBM time; the launch is one chunk of "
@@ -469,7 +469,8 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
                            "tokens_per_s_18_layer_cold_graph": T / (cold_ms * 1e-3), "alg_TFLOPs": flops / (one_ms * 1e-3) / 1e12}
             res["roofline_scan_cold"] = {"kernel": "esc_scan_tc_kernel<128,64,4,float> (B1 H16 d128 T=16448 chunk 64: BASELINE config 2 cold scan, one layer)", "bound": "hbm",
                                     "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": gbs / pk["hbm_gbs"],
-                                    "peak_source": pk["source"], "traffic": 308.4e6, "us_per_launch": one_ms * 1e3,
+                                    "peak_source": pk["source"], "traffic": 311.3e6, "us_per_launch": one_ms * 1e3,
+                                    "traffic_note": "ncu r01u (profiles/r01u_scan_ncu_full.txt): dram read 203.3 MB + write 108.0 MB in the kernel's window",
                                     "alg_bytes_per_launch": alg}
         cold_graph.destroy()
         warm_graph.destroy()
