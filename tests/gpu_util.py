@@ -87,5 +87,39 @@ def err_s(s_gpu, s_ref):
     return float(np.linalg.norm((s_gpu - s_ref).ravel()) / den) if den > 0 else float(np.abs(s_gpu).max())
 
 
+TOL_S_SLICE = 2e-3   # the same ratio over each (b, h, 16-column d_v slice) — the kernels' unit of work
+
+
+def err_s_slices(s_gpu, s_ref, width=16):
+    """max over (b, h, d_v slice of `width` columns) of the relative Frobenius error of that slice: a defect confined
+    to one CTA's slice of one head is not diluted by the rest of the layer."""
+    s_gpu = np.asarray(s_gpu, np.float64)
+    s_ref = np.asarray(s_ref, np.float64)
+    B, H, dk, dv = s_ref.shape
+    w = min(width, dv)
+    d = (s_gpu - s_ref).reshape(B, H, dk, dv // w, w)
+    r = s_ref.reshape(B, H, dk, dv // w, w)
+    num = np.sqrt((d * d).sum(axis=(2, 4)))
+    den = np.sqrt((r * r).sum(axis=(2, 4)))
+    tiny = den <= 0
+    return float(np.where(tiny, num, num / np.where(tiny, 1.0, den)).max())
+
+
+def assert_state_close(s_gpu, s_ref, tag=""):
+    """north_star's state gate (whole-layer relative Frobenius <= 1e-3) plus the per-slice maximum (<= 2e-3)."""
+    s_gpu = s_gpu.cpu().numpy() if hasattr(s_gpu, "cpu") else s_gpu
+    e = err_s(s_gpu, s_ref)
+    assert e <= TOL_S, "S error %.3e %s" % (e, tag)
+    es = err_s_slices(s_gpu, s_ref)
+    assert es <= TOL_S_SLICE, "S per-slice error %.3e %s" % (es, tag)
+
+
+def sample_heads(B, H, n, *seed_ids):
+    """n distinct seeded (b, h) pairs (the full-size tests check a sample of heads against the oracle)."""
+    r = synth.rng(900, *seed_ids)
+    idx = r.choice(B * H, size=min(n, B * H), replace=False)
+    return [(int(i) // H, int(i) % H) for i in idx]
+
+
 def bits_equal(a: torch.Tensor, b: torch.Tensor) -> bool:
     return bool(torch.equal(a.contiguous().view(torch.uint8), b.contiguous().view(torch.uint8)))

@@ -8,7 +8,7 @@ import torch
 
 import oracle
 from paper_2606_20537_b200 import synth
-from gpu_util import DEV, TOL_O, TOL_S, bits_equal, err_o, err_s, esc_mod, scan_dev_inputs, to_dev
+from gpu_util import DEV, TOL_O, TOL_S, assert_state_close, bits_equal, err_o, err_s, esc_mod, sample_heads, scan_dev_inputs, to_dev
 
 pytestmark = pytest.mark.gpu
 
@@ -53,7 +53,7 @@ def test_gdn_vs_oracle(esc, ctx, B, H, dk, dv, T, gate, with_s0):
     q, k, v, g = si.as_f32()
     o_ref, s_ref = oracle.gdn_recurrence(q, k, v, g, beta, None if s0 is None else s0.astype(np.float64))
     assert err_o(o.cpu().numpy(), o_ref) <= TOL_O
-    assert err_s(s.cpu().numpy(), s_ref) <= TOL_S
+    assert_state_close(s, s_ref)
     assert err_o(o.cpu().numpy(), o_ref) <= 5e-5 and err_s(s.cpu().numpy(), s_ref) <= 5e-5   # two-term bf16 operands, fp32 accumulation: far inside the gates
 
 
@@ -98,11 +98,11 @@ def test_gdn_full_size_sampled(esc, ctx):
     si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(73,))
     beta = synth.gdn_beta(B, T, H, seed_ids=(73,))
     o, s, _ = run_gdn(esc, ctx, scan_dev_inputs(si), to_dev(beta), B, T, H, dk, dv)
-    heads = [0, 9, 15]
+    heads = sorted(h for _, h in sample_heads(B, H, 3, 73))
     q, k, v, g = si.as_f32()
     o_ref, s_ref = oracle.gdn_recurrence(q[:, :, heads], k[:, :, heads], v[:, :, heads], g[:, :, heads], beta[:, :, heads])
     assert err_o(o[:, :, heads].cpu().numpy(), o_ref) <= TOL_O
-    assert err_s(s[:, heads].cpu().numpy(), s_ref) <= TOL_S
+    assert_state_close(s[:, heads], s_ref)
 
 
 def test_gdn_errors(esc, ctx):

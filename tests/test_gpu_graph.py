@@ -6,7 +6,8 @@ import torch
 
 import oracle
 from paper_2606_20537_b200 import synth
-from gpu_util import DEV, TOL_O, TOL_S, LiveSet, bits_equal, err_o, err_s, esc_mod, scan_dev_inputs
+from gpu_util import (DEV, TOL_O, TOL_S, LiveSet, assert_state_close, bits_equal, err_o, err_s, esc_mod, sample_heads,
+                      scan_dev_inputs)
 
 pytestmark = pytest.mark.gpu
 
@@ -93,7 +94,7 @@ def test_restore_plus_suffix_scan_graph(esc, ctx):
     q, k, v, g = ins[3].as_f32()
     o_ref, s_ref = oracle.linattn_recurrence(q, k, v, g, s0_a[3].cpu().numpy().astype(np.float64))
     assert err_o(outs[3].cpu().numpy(), o_ref) <= TOL_O
-    assert err_s(states[3].cpu().numpy(), s_ref) <= TOL_S
+    assert_state_close(states[3], s_ref)
     graph.destroy()
 
 
@@ -180,7 +181,93 @@ def test_config3_fork_continue_rollback_replay(esc, ctx):
     qf, kf, vf, gf = si.as_f32()
     o_ref, s_ref = oracle.linattn_recurrence(qf, kf, vf, gf, src.states[5].cpu().numpy().astype(np.float64))
     assert err_o(inputs[3].out[5].cpu().numpy(), o_ref) <= TOL_O
-    assert err_s(second[3][0][5].cpu().numpy(), s_ref) <= TOL_S
+    assert_state_close(second[3][0][5], s_ref)
+
+
+def test_config2_capsule_and_warm_graph_equal_cold_graph(esc, ctx):
+    # BASELINE config 2 end to end at full size (PAPER.md:165 three correctness layers, :223 "chunk-aligned long boundary =
+    # cold full prefill", :243-252 the 16k row of Table 7):
+    #   (1) the 402 MiB capsule at P = 16384: snapshot / restore byte-exact against the memcpy oracle;
+    #   (2) ONE graph [restore(16384) + 18 x scan(64)] after an adversarial dirty is bit-identical to the cold graph
+    #       [18 x scan(16448)] on o[16384:16448] and on all 18 final states;
+    #   (3) one layer against the fp64 oracle on a seeded sample of heads.
+    P, T = 16384, 16384 + SUFFIX
+    live, lin = _hybrid_live(esc, ctx, T, 7)
+    n_lin = len(lin)
+    assert n_lin == 18
+    states = [live.dev[i].view(torch.float32).view(B, H, DK, DV) for i in lin]
+    key = esc.shape_key_make(B, H, DK, DV, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
+    # per-layer inputs: three seeded draws, rolled along T for the other layers (same distribution, distinct per layer)
+    base = [synth.scan_inputs(B, T, H, DK, DV, seed_ids=(25, n)) for n in range(3)]
+    base_dev = [scan_dev_inputs(si) for si in base]
+    shift = lambda n: 0 if n < 3 else 64 * 7 * n       # a multiple of the chunk: the rolled layers stay chunk-aligned
+    dev_ins = [tuple(torch.roll(t, shifts=shift(n), dims=1) for t in base_dev[n % 3]) for n in range(n_lin)]
+    stream = torch.cuda.Stream()
+
+    # ---- cold: 18 x scan(16448) from S_0 = 0 as one graph (the configuration bench.py's warm_vs_cold times) ----
+    s_cold = [torch.full((B, H, DK, DV), float("nan"), dtype=torch.float32, device=DEV) for _ in range(n_lin)]
+    o_cold = [torch.full((B, T, H, DV), float("nan"), dtype=torch.float32, device=DEV) for _ in range(n_lin)]
+    cold = esc.graph_capture(ctx, None, 0, [esc.scan_args(key, *dev_ins[n], None, s_cold[n], o_cold[n], T, T, CHUNK)
+                                            for n in range(n_lin)], stream)
+    cold.launch(stream)
+    stream.synchronize()
+    cold.destroy()
+    o_cold_tail = [o[:, P:].clone() for o in o_cold]
+
+    # ---- prefill to P in the live fold states (S_0 = 0), snapshot: the 402 MiB capsule ----
+    for n in range(n_lin):
+        q, k, v, g = dev_ins[n]
+        esc.linattn_scan(ctx, key, q, k, v, g, None, states[n], o_cold[n], P, T, CHUNK)   # o[:P] rewritten with the same bits
+    torch.cuda.synchronize()
+    for n, i in enumerate(lin):                               # host twin of the fold states for the memcpy oracle
+        live.host[i][:] = live.dev[i].cpu().numpy()
+    live.set.set_position(P)
+    slab_bytes, payload = live.set.capsule_bytes(P)
+    assert payload == 18 * (1 << 20) + 24576 * P == 421527552      # 402 MiB
+    slab = torch.empty(slab_bytes, dtype=torch.uint8, device=DEV)
+    cap = esc.snapshot(live.set, P, CHUNK, slab)
+    torch.cuda.synchronize()
+    ref = oracle.capsule_snapshot(live.oracle_rows(), P)
+    assert np.array_equal(slab.cpu().numpy(), ref), "402 MiB capsule differs from the oracle's memcpy capsule"
+    # restore by the verb after an adversarial dirty: byte-exact on every row, beyond-valid bytes keep the dirt
+    live.fill(26, 0, pattern=0xFF)
+    esc.restore(live.set, cap)
+    oracle.capsule_restore(live.oracle_rows(), P, ref)
+    live.assert_equals_host()
+
+    # ---- warm: ONE graph [restore(16384) + 18 x scan(64)] ----
+    o_warm = [torch.full((B, SUFFIX, H, DV), float("nan"), dtype=torch.float32, device=DEV) for _ in range(n_lin)]
+    layers = []
+    for n in range(n_lin):
+        q, k, v, g = dev_ins[n]
+        layers.append(esc.scan_args(key, q[:, P:], k[:, P:], v[:, P:], g[:, P:], states[n], states[n], o_warm[n],
+                                    SUFFIX, T, CHUNK))
+    warm = esc.graph_capture(ctx, live.set, P, layers, stream)
+    live.fill(27, 0, pattern=0xFF)
+    torch.cuda.synchronize()
+    warm.set_capsule(cap, stream)
+    warm.launch(stream)
+    stream.synchronize()
+    for n in range(n_lin):
+        assert bits_equal(o_warm[n], o_cold_tail[n]), "layer %d: warm o[16384:] differs from the cold graph" % n
+        assert bits_equal(states[n], s_cold[n]), "layer %d: warm S_16448 differs from the cold graph" % n
+    # KV rows: valid ranges restored byte-exactly (the oracle's memcpy twin), beyond-valid bytes still dirty
+    oracle.capsule_restore(live.oracle_rows(), P, ref)
+    for i, spec in enumerate(live.specs):
+        if spec.bytes_per_token:
+            assert np.array_equal(live.dev[i].cpu().numpy(), live.host[i]), spec.name
+    warm.destroy()
+    cap.destroy()
+
+    # ---- one layer against the oracle (seeded sample of heads, whole 16448-token sequence) ----
+    n = 1
+    q, k, v, g = base[n].as_f32()
+    for (b, h) in sample_heads(B, H, 3, 25):
+        sl = (slice(b, b + 1), slice(None), slice(h, h + 1))
+        o_ref, s_ref = oracle.linattn_recurrence(q[sl], k[sl], v[sl], g[sl])
+        assert err_o(o_warm[n][b:b + 1, :, h:h + 1].cpu().numpy(), o_ref[:, P:]) <= TOL_O
+        assert err_o(o_cold[n][b:b + 1, :, h:h + 1].cpu().numpy(), o_ref) <= TOL_O
+        assert_state_close(states[n][b:b + 1, h:h + 1], s_ref)
 
 
 def test_plan_table_lru_and_padded_bucket(esc):

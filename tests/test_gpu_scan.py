@@ -10,7 +10,8 @@ import torch
 
 import oracle
 from paper_2606_20537_b200 import synth
-from gpu_util import DEV, TOL_O, TOL_S, bits_equal, err_o, err_s, esc_mod, scan_dev_inputs, to_dev
+from gpu_util import (DEV, TOL_O, TOL_S, assert_state_close, bits_equal, err_o, err_s, esc_mod, sample_heads,
+                      scan_dev_inputs, to_dev)
 
 pytestmark = pytest.mark.gpu
 
@@ -67,9 +68,9 @@ def test_scan_vs_oracle(esc, ctx, B, H, dk, dv, T, chunk, gate, with_s0):
     dev_in = scan_dev_inputs(si)
     o, s, o_full = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, None if s0_np is None else to_dev(s0_np))
     assert not torch.isnan(o).any() and not torch.isnan(s).any()
-    eo, es = err_o(o.cpu().numpy(), o_ref), err_s(s.cpu().numpy(), s_ref)
+    eo = err_o(o.cpu().numpy(), o_ref)
     assert eo <= TOL_O, "o error %.3e" % eo
-    assert es <= TOL_S, "S error %.3e" % es
+    assert_state_close(s, s_ref)
     # bf16-o variant: RNE of the fp32 kernel's result, state identical
     o16, s16, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, None if s0_np is None else to_dev(s0_np),
                            out_bf16=True)
@@ -92,7 +93,8 @@ def test_batch_stride_and_untouched_tail(esc, ctx):
     si = synth.scan_inputs(B, Tbuf, H, dk, dv, seed_ids=(12,))
     o_ref, s_ref = oracle.linattn_recurrence(*si.as_f32(), T=T)
     o, s, o_full = run_scan(esc, ctx, scan_dev_inputs(si), B, T, H, dk, dv, 64, n=T)
-    assert err_o(o.cpu().numpy(), o_ref) <= TOL_O and err_s(s.cpu().numpy(), s_ref) <= TOL_S
+    assert err_o(o.cpu().numpy(), o_ref) <= TOL_O
+    assert_state_close(s, s_ref)
     assert torch.isnan(o_full[:, T:]).all(), "tokens beyond T were written"
 
 
@@ -138,7 +140,8 @@ def test_misaligned_restore_is_within_tolerance(esc, ctx):
     o_a, s_p, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, n=P)
     o_b, s_t, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=s_p, t0=P)
     o = torch.cat([o_a, o_b], dim=1)
-    assert err_o(o.cpu().numpy(), o_ref) <= TOL_O and err_s(s_t.cpu().numpy(), s_ref) <= TOL_S
+    assert err_o(o.cpu().numpy(), o_ref) <= TOL_O
+    assert_state_close(s_t, s_ref)
 
 
 def test_kv_only_restore_diverges(esc, ctx):
@@ -177,51 +180,54 @@ def test_scan_argument_errors(esc, ctx):
     assert e.value.code == esc.ERR_INVALID
 
 
+def _check_sampled_heads(si, o, s, pairs, t_from=0):
+    """oracle over the whole sequence for each sampled (b, h); compares o[:, t_from:] and the final state."""
+    q, k, v, g = si.as_f32()
+    for (b, h) in pairs:
+        sl = (slice(b, b + 1), slice(None), slice(h, h + 1))
+        o_ref, s_ref = oracle.linattn_recurrence(q[sl], k[sl], v[sl], g[sl])
+        eo = err_o(o[b:b + 1, :, h:h + 1].cpu().numpy(), o_ref[:, t_from:])
+        assert eo <= TOL_O, "o error %.3e at (b, h) = %s" % (eo, (b, h))
+        assert_state_close(s[b:b + 1, h:h + 1], s_ref, "at (b, h) = %s" % ((b, h),))
+
+
 def test_full_size_config2_sampled(esc, ctx):
     # BASELINE config 2's cold scan at full size (B1 H16 d128, T = 16384 + 64, chunk 64) in the launch
     # configuration bench.py times; the oracle checks a seeded sample of heads over the whole sequence.
     B, H, dk, dv, T, chunk = 1, 16, 128, 128, 16384 + 64, 64
     si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(16,))
     o, s, _ = run_scan(esc, ctx, scan_dev_inputs(si), B, T, H, dk, dv, chunk)
-    heads = [0, 7, 15]
-    q, k, v, g = si.as_f32()
-    o_ref, s_ref = oracle.linattn_recurrence(q[:, :, heads], k[:, :, heads], v[:, :, heads], g[:, :, heads])
-    assert err_o(o[:, :, heads].cpu().numpy(), o_ref) <= TOL_O
-    assert err_s(s[:, heads].cpu().numpy(), s_ref) <= TOL_S
+    _check_sampled_heads(si, o, s, sample_heads(B, H, 3, 16))
 
 
 @pytest.mark.parametrize("B,T,chunk", [
-    (4, 2048, 64),      # 64 (b,h) scans = 128 clusters: several waves of CTAs on 148 SMs
+    (4, 2048, 64),      # 64 (b,h) scans: several waves of CTAs on 148 SMs
     (2, 8192, 128),
+    (4, 8192, 64),      # the B = 4 tile at a length bench.py times
     (1, 32768, 64),
+    (1, 65536, 64),     # 1024 chunks: every barrier parity wraps 256+ times, the gate warp batches 256 times
+    (4, 32768, 64),     # the largest B x T bench.py's sweep times
 ])
 def test_config4_sweep_points_sampled(esc, ctx, B, T, chunk):
-    # BASELINE config 4 (scan sweep: B 1-4, H16, d128, T 2k-64k, chunk 64/128) at full head shape: the oracle checks a
+    # BASELINE config 4 (scan sweep: B 1-4, H16, d128, T 2k-64k, chunk 64/128) at full head shape, every (B, T) the
+    # bench's scan_sweep publishes a number for that the three historical points did not cover: the oracle checks a
     # seeded sample of (b, h) scans over the whole sequence; a chunk-aligned boundary at T/2 must continue bit-identically
     # to the cold run, a misaligned one (T/2 + 37) within tolerance.
     H, dk, dv = 16, 128, 128
     si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(17, B, T, chunk))
     dev_in = scan_dev_inputs(si)
     o_cold, s_cold, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk)
-    q, k, v, g = si.as_f32()
-    for (b, h) in [(0, 0), (B - 1, 9), (B // 2, 15)]:
-        sl = (slice(b, b + 1), slice(None), slice(h, h + 1))
-        o_ref, s_ref = oracle.linattn_recurrence(q[sl], k[sl], v[sl], g[sl])
-        assert err_o(o_cold[b:b + 1, :, h:h + 1].cpu().numpy(), o_ref) <= TOL_O
-        assert err_s(s_cold[b:b + 1, h:h + 1].cpu().numpy(), s_ref) <= TOL_S
-        # misaligned restore of this (b, h): oracle tolerance only
+    pairs = sample_heads(B, H, 3, 17, B, T, chunk)
+    _check_sampled_heads(si, o_cold, s_cold, pairs)
     P = (T // 2) // chunk * chunk
     _, s_p, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, n=P)
     o_b, s_t, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=s_p, t0=P)
     assert bits_equal(o_b, o_cold[:, P:]) and bits_equal(s_t, s_cold)
+    del o_b, s_t
     Pm = P + 37
     _, s_pm, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, n=Pm)
     o_m, s_tm, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=s_pm, t0=Pm)
-    b, h = B - 1, 9
-    sl = (slice(b, b + 1), slice(None), slice(h, h + 1))
-    o_ref, s_ref = oracle.linattn_recurrence(q[sl], k[sl], v[sl], g[sl])
-    assert err_o(o_m[b:b + 1, :, h:h + 1].cpu().numpy(), o_ref[:, Pm:]) <= TOL_O
-    assert err_s(s_tm[b:b + 1, h:h + 1].cpu().numpy(), s_ref) <= TOL_S
+    _check_sampled_heads(si, o_m, s_tm, pairs[:1], t_from=Pm)   # misaligned restore: oracle tolerance only
 
 
 def test_back_to_back_scans_on_one_stream_are_ordered(esc, ctx):
@@ -283,7 +289,7 @@ def test_seeded_shape_fuzz_vs_oracle(esc, ctx):
         o_ref, s_ref = oracle.linattn_recurrence(*si.as_f32(), None if s0 is None else s0.astype(np.float64))
         tag = (it, B, H, dk, dv, T, chunk, gate)
         assert err_o(o.cpu().numpy(), o_ref) <= TOL_O, tag
-        assert err_s(s.cpu().numpy(), s_ref) <= TOL_S, tag
+        assert_state_close(s, s_ref, str(tag))
         P = (T // 2) // chunk * chunk
         if P > 0:
             _, s_p, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk, s0=None if s0 is None else to_dev(s0), n=P)

@@ -110,10 +110,45 @@ def test_causal_conv_is_an_fir_filter(W):
             np.testing.assert_allclose(y[b, :, c], ref, rtol=1e-12, atol=1e-14)
     if W > 1:
         np.testing.assert_array_equal(st, np.transpose(x[:, T - (W - 1):, :], (0, 2, 1)).astype(np.float64))
-    # continuation with the carried window == one run, bitwise; SiLU is y / (1 + exp(-y))
+    # continuation with the carried window == one run, bitwise
     for P in (1, 2, 20):
         y1, s1 = oracle.causal_conv(x, w, T=P)
         y2, s2 = oracle.causal_conv(x[:, P:], w, s1)
         assert np.array_equal(np.concatenate([y1, y2], axis=1), y) and np.array_equal(s2, st)
+
+
+def test_causal_conv_silu_branch_is_pinned():
+    """The SiLU branch of the convolution oracle against things the mathematics fixes (not its own formula):
+    the library logistic function scipy.special.expit, hand values, the odd-part identity silu(y) - silu(-y) = y,
+    silu(0) = 0, the large-|y| limits, and the derivative at 0 (1/2) by a central difference."""
+    # W = 1 with unit taps makes the pre-activation the input itself: y = x exactly, so known arguments can be fed in
+    pts = np.array([0.0, 1.0, -1.0, 2.0, -2.0, 0.5, 30.0, -30.0, 1e-4, -1e-4], np.float32)
+    x = pts[None, :, None]
+    w = np.ones((1, 1), np.float32)
+    y_lin, _ = oracle.causal_conv(x, w)
+    np.testing.assert_array_equal(y_lin[0, :, 0], pts.astype(np.float64))
     ys, _ = oracle.causal_conv(x, w, silu=True)
-    np.testing.assert_allclose(ys, y / (1.0 + np.exp(-y)), rtol=1e-15)
+    s = dict(zip(pts.tolist(), ys[0, :, 0].tolist()))
+    # hand values: silu(1) = 1 / (1 + e^-1), silu(-1) = -1 / (1 + e), silu(2) = 2 / (1 + e^-2)
+    assert s[0.0] == 0.0
+    assert abs(s[1.0] - 0.7310585786300049) < 1e-15
+    assert abs(s[-1.0] + 0.2689414213699951) < 1e-15
+    assert abs(s[2.0] - 1.7615941559557649) < 1e-15
+    # odd part: silu(y) - silu(-y) = y (sigmoid(y) + sigmoid(-y) = 1)
+    for a in (1.0, 2.0, 30.0, float(np.float32(1e-4))):
+        assert abs((s[a] - s[-a]) - a) < 1e-14 * max(1.0, a)
+    # limits: silu(y) -> y for large y, -> 0- for very negative y
+    assert abs(s[30.0] - 30.0) < 1e-11 and -1e-11 < s[-30.0] < 0.0
+    # slope 1/2 at the origin
+    h = float(np.float32(1e-4))
+    assert abs((s[h] - s[-h]) / (2 * h) - 0.5) < 1e-12
+    # against the library logistic function on a real convolution (W = 4, random taps and inputs)
+    import scipy.special
+    r = np.random.default_rng([7, 99])
+    x = r.standard_normal((2, 33, 5)).astype(np.float32) * 3
+    w = r.standard_normal((5, 4)).astype(np.float32)
+    y, _ = oracle.causal_conv(x, w)
+    ys, st = oracle.causal_conv(x, w, silu=True)
+    np.testing.assert_allclose(ys, y * scipy.special.expit(y), rtol=1e-14, atol=1e-300)
+    # the activation does not touch the carried window
+    np.testing.assert_array_equal(st, oracle.causal_conv(x, w)[1])
