@@ -22,8 +22,14 @@
  *   - "dev" pointers are CUDA device pointers, "host" pointers are ordinary host memory.
  *   - Ownership: the library NEVER allocates or frees tensor memory.  Live buffers and
  *     capsule storage slabs are caller-owned device memory (the Python binding uses
- *     torch tensors).  The library owns only its small host structs and, per esc_graph,
- *     one device-resident descriptor table (a few KiB), rewritten by a one-CTA kernel.
+ *     torch tensors), and so is the few-KiB device scratch an esc_graph keeps its
+ *     "current capsule" descriptor table in (esc_graph_scratch_bytes).  The library owns
+ *     only its small host structs.
+ *   - Devices: a handle belongs to its context's device.  Every verb runs on that device
+ *     whatever the calling thread's current device is and leaves the current device as it
+ *     found it; kernel attributes are tracked per context, so several contexts (one per GPU)
+ *     may live in one process.  A context may be used from several host threads as long as
+ *     calls on the same live set / graph / plan table are serialised by the caller.
  *   - Streams: every verb only ENQUEUES work on the caller's cudaStream_t (passed as
  *     void*; NULL = legacy default stream) and returns without a host sync.  Everything
  *     the host can detect (bad arguments, layout / digest mismatch, unaligned boundary,
@@ -40,7 +46,7 @@
 extern "C" {
 #endif
 
-#define ESC_ABI_VERSION 1u
+#define ESC_ABI_VERSION 2u
 
 /* ---- error codes -------------------------------------------------------------------- */
 #define ESC_OK               0
@@ -103,7 +109,7 @@ typedef struct esc_buf_desc {
 int esc_bufset_create(esc_ctx* ctx, const esc_buf_desc* descs, uint32_t n_rows, esc_bufset** out_set);
 /* Destroy a live set or a capsule handle (never frees device memory). */
 int esc_bufset_destroy(esc_bufset* set);
-/* FNV-1a-64 over (ABI version, row names, fixed_bytes, bytes_per_token, n_seg): two sets
+/* FNV-1a-64 over (layout version, row names, fixed_bytes, bytes_per_token, n_seg): two sets
  * with the same digest have the same capsule layout (pointers, capacities and strides are
  * not part of it).  PAPER.md:121,124 "digest". */
 int esc_bufset_layout_digest(const esc_bufset* set, uint64_t* out_digest);
@@ -303,13 +309,22 @@ typedef struct esc_scan_args {
 /*
  * Capture ONE CUDA graph = [restore node: capsule -> `live`] -> [scan node per layer, in
  * order].  `live` may be NULL (no restore node: a cold plan).  The restore node reads its
- * copy table from a device-resident descriptor owned by the graph, so the capsule can be
- * swapped between replays WITHOUT recapturing (the paper's "host overwrites a bound
- * sub-buffer between replays" idiom).  `max_boundary` bounds the capsules
- * that may later be bound (sizes the persistent grid).  `stream` is used for the capture.
+ * copy table from a device-resident descriptor, so the capsule can be swapped between replays
+ * WITHOUT recapturing (the paper's "host overwrites a bound sub-buffer between replays" idiom,
+ * PAPER.md:110).  That descriptor lives in `scratch_dev`: caller-owned device memory of at least
+ * esc_graph_scratch_bytes() bytes, 16-byte aligned (ESC_ERR_CAPACITY / ESC_ERR_UNALIGNED), which
+ * must stay allocated, and untouched by the caller, until the graph is destroyed; a cold plan
+ * (live == NULL) takes NULL / 0.  `max_boundary` bounds the capsules that may later be bound
+ * (it sizes the restore node's grid; esc_graph_set_capsule refuses a later boundary with
+ * ESC_ERR_CAPACITY).  `stream` is used for the capture and for one small kernel ahead of it that
+ * stores an empty table (a launch before any capsule is bound is refused on the host anyway).
+ * Lifetimes: `live`, the layers' buffers and the scratch are referenced, not copied — they must
+ * outlive the graph (destroy the graph before the live set).
  */
+uint64_t esc_graph_scratch_bytes(void);
 int esc_graph_capture(esc_ctx* ctx, esc_bufset* live, uint64_t max_boundary,
-                      const esc_scan_args* layers, uint32_t n_layers, void* stream, esc_graph** out_graph);
+                      const esc_scan_args* layers, uint32_t n_layers,
+                      void* scratch_dev, uint64_t scratch_bytes, void* stream, esc_graph** out_graph);
 /* Bind the capsule the next launches restore from: host rebuilds the table and enqueues one
  * small kernel on `stream` that stores it to the graph's device-resident copy (the table travels as a
  * kernel parameter: no copy engine, no host-side wait; the call may be repeated at any rate).  Same layout / capacity checks as esc_restore. */
@@ -317,6 +332,7 @@ int esc_graph_set_capsule(esc_graph* graph, const esc_bufset* capsule, void* str
 /* One cudaGraphLaunch on `stream`.  ESC_ERR_INVALID if the plan has a restore node and no
  * capsule is bound. */
 int esc_graph_launch(esc_graph* graph, void* stream);
+/* ESC_ERR_INVALID for a plan the context's Graph[key] table owns (the table destroys it on eviction / esc_ctx_destroy). */
 int esc_graph_destroy(esc_graph* graph);
 
 /* ---- Graph[key] table ("replay Graph[key]"; "a bounded set of shape variants
@@ -327,8 +343,11 @@ int esc_graph_destroy(esc_graph* graph);
  *       any suffix T' <= bucket whose tail the caller pads with k = v = 0, g = 1 tokens (reading 13: the state
  *       and the real tokens' outputs are bit-identical to a T'-token scan, the chunk grid being the same).
  *   esc_plan_key_make(shape key, suffix bucket, max boundary, n_layers): opaque 64-bit key (FNV-1a of the four).
- *   put: the table takes ownership of `graph`; inserting into a full table destroys the least recently used plan;
- *        putting an existing key replaces (and destroys) the old plan.  capacity >= 1 (default 8).
+ *   put: the table takes ownership of `graph` (esc_graph_destroy on it then fails); inserting into a full table destroys
+ *        the least recently used plan; putting an existing key replaces (and destroys) the old plan; a graph already held
+ *        under another key is refused (ESC_ERR_INVALID).  capacity >= 1 (default 8).
+ *   contains: whether a key is present, without touching the LRU order or the statistics (lets a binding drop its
+ *        references to evicted plans).
  *   get: ESC_OK and the plan (now most recently used), or ESC_ERR_MISMATCH when the key is absent — "a new shape
  *        needing capture": the caller captures and puts.  The table still owns the plan.
  *   stats: hits, misses, evictions since the context was created. */
@@ -337,6 +356,7 @@ uint64_t esc_plan_key_make(esc_shape_key key, uint64_t suffix_bucket, uint64_t m
 int esc_plan_table_set_capacity(esc_ctx* ctx, uint32_t capacity);
 int esc_plan_table_put(esc_ctx* ctx, uint64_t plan_key, esc_graph* graph);
 int esc_plan_table_get(esc_ctx* ctx, uint64_t plan_key, esc_graph** out_graph);
+int esc_plan_table_contains(const esc_ctx* ctx, uint64_t plan_key, uint32_t* out_present);
 int esc_plan_table_stats(const esc_ctx* ctx, uint32_t* out_size, uint64_t* out_hits, uint64_t* out_misses,
                          uint64_t* out_evictions);
 

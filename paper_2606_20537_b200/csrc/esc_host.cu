@@ -53,17 +53,62 @@ static uint64_t fnv1a(uint64_t h, const void* p, size_t n) {
     return h;
 }
 
-static uint64_t layout_digest(const std::vector<Row>& rows) {
+// The digest identifies the capsule LAYOUT (reading 16 of DESIGN.md), not the library build: its version word is the layout
+// version, which changes only when the slab layout contract of include/esc.h does.
+static const uint32_t kLayoutVersion = 1;
+
+static uint64_t layout_digest(const std::vector<Row>& rows, const std::vector<std::string>& names) {
     uint64_t h = 0xcbf29ce484222325ull;
-    const uint32_t abi = ESC_ABI_VERSION;
-    h = fnv1a(h, &abi, sizeof abi);
-    for (const Row& r : rows) {
-        h = fnv1a(h, r.name.data(), r.name.size() + 1);
+    h = fnv1a(h, &kLayoutVersion, sizeof kLayoutVersion);
+    for (size_t i = 0; i < rows.size(); ++i) {
+        const Row& r = rows[i];
+        h = fnv1a(h, names[i].data(), names[i].size() + 1);
         h = fnv1a(h, &r.fixed_bytes, 8);
         h = fnv1a(h, &r.bytes_per_token, 8);
         h = fnv1a(h, &r.n_seg, 4);
     }
     return h;
+}
+
+const SegCache& live_segs(esc_bufset* live, uint64_t P) {
+    SegCache& c = live->seg_cache;
+    if (!c.valid || c.P != P) {
+        layout_walk(live->rows, P, &c.segs, &c.slab_bytes, &c.payload_bytes);
+        c.P = P;
+        c.valid = true;
+    }
+    return c;
+}
+
+void build_restore_table(CopyTable* t, const std::vector<Seg>& segs, const uint8_t* slab) {
+    const uint8_t* src[kCopyMaxSeg];
+    uint8_t* dst[kCopyMaxSeg];
+    uint64_t bytes[kCopyMaxSeg];
+    const uint32_t n = (uint32_t)segs.size();   // callers check n <= kCopyMaxSeg
+    for (uint32_t i = 0; i < n; ++i) {
+        src[i] = slab + segs[i].slab_off;
+        dst[i] = segs[i].live;
+        bytes[i] = segs[i].bytes;
+    }
+    build_copy_table(t, src, dst, bytes, n);
+}
+
+int launch_copy_segs(const esc_ctx* ctx, const std::vector<Seg>& segs, uint8_t* slab, bool to_slab, cudaStream_t stream) {
+    const uint8_t* src[kCopyMaxSeg];
+    uint8_t* dst[kCopyMaxSeg];
+    uint64_t bytes[kCopyMaxSeg];
+    for (size_t first = 0; first < segs.size(); first += kCopyMaxSeg) {
+        const uint32_t m = (uint32_t)(segs.size() - first < kCopyMaxSeg ? segs.size() - first : kCopyMaxSeg);
+        for (uint32_t i = 0; i < m; ++i) {
+            const Seg& sg = segs[first + i];
+            src[i] = to_slab ? sg.live : slab + sg.slab_off;
+            dst[i] = to_slab ? slab + sg.slab_off : sg.live;
+            bytes[i] = sg.bytes;
+        }
+        int rc = launch_copy(ctx, src, dst, bytes, m, stream);
+        if (rc != ESC_OK) return rc;
+    }
+    return ESC_OK;
 }
 
 // Pair a capsule with a live set: same layout digest, every valid range fits the live buffers.
@@ -103,10 +148,17 @@ int esc_ctx_create(int device, esc_ctx** out_ctx) {
     cudaDeviceProp p;
     ESC_CUDA(cudaGetDeviceProperties(&p, device));
     if (p.major != 10) return ESC_ERR_UNSUPPORTED;  // sm_100a SASS only, no fallback
-    ESC_CUDA(cudaSetDevice(device));
     esc_ctx* c = new (std::nothrow) esc_ctx;
     if (!c) return ESC_ERR_INVALID;
     c->device = device;
+    {   // create the device's primary context now (first use), leaving the caller's current device alone
+        DeviceGuard g(c);
+        cudaError_t e = g.err == cudaSuccess ? cudaFree(nullptr) : g.err;
+        if (e != cudaSuccess) {
+            delete c;
+            return cuda_fail(e);
+        }
+    }
     c->sm_count = p.multiProcessorCount;
     c->l2_bytes = p.l2CacheSize;
     *out_ctx = c;
@@ -115,6 +167,7 @@ int esc_ctx_create(int device, esc_ctx** out_ctx) {
 
 int esc_ctx_destroy(esc_ctx* ctx) {
     if (!ctx) return ESC_ERR_INVALID;
+    ESC_ON_DEVICE(ctx);
     free_plan_table(ctx);   // the Graph[key] table owns its plans
     delete ctx;
     return ESC_OK;
@@ -130,13 +183,15 @@ int esc_bufset_create(esc_ctx* ctx, const esc_buf_desc* descs, uint32_t n_rows, 
     if (!ctx || !descs || !out_set || n_rows == 0 || n_rows > ESC_MAX_ROWS) return ESC_ERR_INVALID;
     std::vector<Row> rows;
     rows.reserve(n_rows);
+    auto names = std::make_shared<std::vector<std::string>>();
+    names->reserve(n_rows);
     for (uint32_t i = 0; i < n_rows; ++i) {
         const esc_buf_desc& d = descs[i];
         if (!d.name || !d.dev_ptr || d.n_seg == 0 || d.reserved != 0) return ESC_ERR_INVALID;
         if (d.fixed_bytes == 0 && d.bytes_per_token == 0) return ESC_ERR_INVALID;
         if (d.n_seg > 1 && d.seg_stride == 0) return ESC_ERR_INVALID;
         Row r;
-        r.name = d.name;
+        names->push_back(d.name);
         r.base = (uint8_t*)d.dev_ptr;
         r.capacity = d.capacity_bytes;
         r.fixed_bytes = d.fixed_bytes;
@@ -151,7 +206,8 @@ int esc_bufset_create(esc_ctx* ctx, const esc_buf_desc* descs, uint32_t n_rows, 
     s->ctx = ctx;
     s->frozen = false;
     s->rows.swap(rows);
-    s->layout_digest = layout_digest(s->rows);
+    s->layout_digest = layout_digest(s->rows, *names);
+    s->names = names;
     s->position = ESC_POSITION_UNKNOWN;
     s->slab = nullptr;
     s->slab_host = nullptr;
@@ -211,16 +267,16 @@ int esc_snapshot(esc_bufset* live, uint64_t P, uint64_t chunk, uint64_t prefix_d
     if (((uintptr_t)storage_dev & 255u) != 0) return ESC_ERR_UNALIGNED;
     int rc = check_fit(live->rows, P);
     if (rc != ESC_OK) return rc;
-    std::vector<Seg> segs;
-    uint64_t slab_bytes = 0, payload = 0;
-    layout_walk(live->rows, P, &segs, &slab_bytes, &payload);
-    if (slab_bytes > storage_bytes) return ESC_ERR_CAPACITY;
+    ESC_ON_DEVICE(live->ctx);
+    const SegCache& sc = live_segs(live, P);
+    if (sc.slab_bytes > storage_bytes) return ESC_ERR_CAPACITY;
 
     esc_bufset* cap = new (std::nothrow) esc_bufset;
     if (!cap) return ESC_ERR_INVALID;
     cap->ctx = live->ctx;
     cap->frozen = true;
-    cap->rows = live->rows;
+    cap->rows = live->rows;       // plain data; the names are shared, not copied
+    cap->names = live->names;
     for (Row& r : cap->rows) {   // a capsule carries the layout (and the stages' valid ends), not the live pointers
         r.base = nullptr;
         r.stage = nullptr;
@@ -230,20 +286,12 @@ int esc_snapshot(esc_bufset* live, uint64_t P, uint64_t chunk, uint64_t prefix_d
     cap->slab = (uint8_t*)storage_dev;
     cap->slab_host = nullptr;
     cap->tier = ESC_TIER_GPU;
-    cap->slab_bytes = slab_bytes;
-    cap->payload_bytes = payload;
+    cap->slab_bytes = sc.slab_bytes;
+    cap->payload_bytes = sc.payload_bytes;
     cap->chunk = chunk;
     cap->prefix_digest = prefix_digest;
 
-    std::vector<const uint8_t*> src(segs.size());
-    std::vector<uint8_t*> dst(segs.size());
-    std::vector<uint64_t> bytes(segs.size());
-    for (size_t i = 0; i < segs.size(); ++i) {
-        src[i] = segs[i].live;
-        dst[i] = cap->slab + segs[i].slab_off;
-        bytes[i] = segs[i].bytes;
-    }
-    rc = launch_copy(live->ctx, src.data(), dst.data(), bytes.data(), (uint32_t)segs.size(), (cudaStream_t)stream);
+    rc = launch_copy_segs(live->ctx, sc.segs, cap->slab, true, (cudaStream_t)stream);
     if (rc != ESC_OK) {
         delete cap;
         return rc;
@@ -253,21 +301,21 @@ int esc_snapshot(esc_bufset* live, uint64_t P, uint64_t chunk, uint64_t prefix_d
 }
 
 static int restore_impl(esc_bufset* live, const esc_bufset* cap, cudaStream_t stream, bool eager_dequant = false) {
-    std::vector<Seg> segs;
-    layout_walk(live->rows, cap->position, &segs, nullptr, nullptr);
-    std::vector<const uint8_t*> src(segs.size());
-    std::vector<uint8_t*> dst(segs.size());
-    std::vector<uint64_t> bytes(segs.size());
-    for (size_t i = 0; i < segs.size(); ++i) {
-        src[i] = cap->slab + segs[i].slab_off;
-        dst[i] = segs[i].live;
-        bytes[i] = segs[i].bytes;
-    }
+    ESC_ON_DEVICE(live->ctx);
+    const std::vector<Seg>& segs = live_segs(live, cap->position).segs;
     int rc;
     if (!eager_dequant) {
-        rc = launch_copy(live->ctx, src.data(), dst.data(), bytes.data(), (uint32_t)segs.size(), stream);
+        rc = launch_copy_segs(live->ctx, segs, cap->slab, false, stream);
         if (rc == ESC_OK) reset_stage_valid(live, 0);   // "rebuilt lazily on the next read, not eagerly in restore"
     } else {
+        std::vector<const uint8_t*> src(segs.size());
+        std::vector<uint8_t*> dst(segs.size());
+        std::vector<uint64_t> bytes(segs.size());
+        for (size_t i = 0; i < segs.size(); ++i) {
+            src[i] = cap->slab + segs[i].slab_off;
+            dst[i] = segs[i].live;
+            bytes[i] = segs[i].bytes;
+        }
         // same walk order as layout_walk: rows in table order, segments inside a row
         std::vector<uint8_t*> d16(segs.size(), nullptr);
         std::vector<float> scale(segs.size(), 1.f);
@@ -316,17 +364,18 @@ int esc_fork(const esc_bufset* capsule, esc_bufset* const* lives, uint32_t n, vo
         for (uint32_t e = 0; e < d; ++e)
             if (lives[e] == lives[d]) return ESC_ERR_INVALID;
     }
-    std::vector<std::vector<Seg>> segs(n);
-    for (uint32_t d = 0; d < n; ++d) layout_walk(lives[d]->rows, capsule->position, &segs[d], nullptr, nullptr);
-    const size_t ns = segs[0].size();
+    ESC_ON_DEVICE(capsule->ctx);
+    std::vector<const std::vector<Seg>*> segp(n);
+    for (uint32_t d = 0; d < n; ++d) segp[d] = &live_segs(lives[d], capsule->position).segs;
+    const size_t ns = segp[0]->size();
     std::vector<const uint8_t*> src(ns);
     std::vector<uint64_t> bytes(ns);
     std::vector<std::vector<uint8_t*>> dst(n, std::vector<uint8_t*>(ns));
     std::vector<uint8_t* const*> dstp(n);
     for (size_t i = 0; i < ns; ++i) {
-        src[i] = capsule->slab + segs[0][i].slab_off;
-        bytes[i] = segs[0][i].bytes;
-        for (uint32_t d = 0; d < n; ++d) dst[d][i] = segs[d][i].live;
+        src[i] = capsule->slab + (*segp[0])[i].slab_off;
+        bytes[i] = (*segp[0])[i].bytes;
+        for (uint32_t d = 0; d < n; ++d) dst[d][i] = (*segp[d])[i].live;
     }
     for (uint32_t d = 0; d < n; ++d) dstp[d] = dst[d].data();
     int rc = launch_fork(capsule->ctx, src.data(), dstp.data(), n, bytes.data(), (uint32_t)ns, (cudaStream_t)stream);
@@ -368,6 +417,7 @@ int esc_capsule_demote(const esc_bufset* capsule, void* storage_host, uint64_t s
         return ESC_ERR_INVALID;
     if (storage_bytes < capsule->slab_bytes) return ESC_ERR_CAPACITY;
     if (((uintptr_t)storage_host & 255u) != 0) return ESC_ERR_UNALIGNED;
+    ESC_ON_DEVICE(capsule->ctx);
     // the storage must be pinned and mapped: the restore kernels read it in place
     cudaPointerAttributes at;
     ESC_CUDA(cudaPointerGetAttributes(&at, storage_host));
@@ -394,6 +444,7 @@ int esc_capsule_promote(const esc_bufset* host_capsule, void* storage_dev, uint6
         return ESC_ERR_INVALID;
     if (storage_bytes < host_capsule->slab_bytes) return ESC_ERR_CAPACITY;
     if (((uintptr_t)storage_dev & 255u) != 0) return ESC_ERR_UNALIGNED;
+    ESC_ON_DEVICE(host_capsule->ctx);
     cudaPointerAttributes at;
     ESC_CUDA(cudaPointerGetAttributes(&at, storage_dev));
     if (at.type != cudaMemoryTypeDevice) return ESC_ERR_INVALID;

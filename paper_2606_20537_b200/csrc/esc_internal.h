@@ -3,6 +3,8 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <atomic>
+#include <memory>
 #include <string>
 #include <utility>
 #include <vector>
@@ -55,8 +57,7 @@ struct ForkTable {                                    // n_dst destinations (lar
 };
 
 // ---- handles ----------------------------------------------------------------------------
-struct Row {
-    std::string name;
+struct Row {                          // plain data: copying a row table allocates nothing (names live in esc_bufset::names)
     uint8_t* base;
     uint64_t capacity, fixed_bytes, bytes_per_token, seg_stride;
     uint32_t n_seg;
@@ -74,16 +75,34 @@ struct esc_ctx {
     int device;
     int sm_count;
     int l2_bytes;
+    // kernel instantiations whose max-dynamic-shared-memory attribute has been set on THIS context's device (the attribute
+    // is per device; a process-wide flag would leave a second context's device at the 48 KiB default)
+    std::atomic<uint64_t> func_attr_mask{0};
     // Graph[key] table (include/esc.h): most recently used first
     std::vector<std::pair<uint64_t, esc_graph*>> plans;
     uint32_t plan_capacity = 8;
     uint64_t plan_hits = 0, plan_misses = 0, plan_evictions = 0;
 };
 
+namespace esc {
+struct Seg {                          // host-side flattened (row, segment) of a live<->slab pairing
+    uint8_t* live;
+    uint64_t slab_off;
+    uint64_t bytes;
+};
+struct SegCache {                     // the flattened segment table of a live set at one boundary (hot path: no rebuild per verb)
+    bool valid = false;
+    uint64_t P = 0, slab_bytes = 0, payload_bytes = 0;
+    std::vector<Seg> segs;
+};
+}  // namespace esc
+
 struct esc_bufset {
     esc_ctx* ctx;
     bool frozen;                      // false: live set; true: capsule
     std::vector<esc::Row> rows;       // live: the registered buffers.  capsule: layout copy (base = nullptr)
+    std::shared_ptr<const std::vector<std::string>> names;   // row names, shared between a live set and its capsules
+    esc::SegCache seg_cache;          // live sets: last boundary walked (snapshot / restore / fork / set_capsule)
     uint64_t layout_digest;
     uint64_t position;                // live: current token position; capsule: boundary P'
     // capsule only
@@ -95,17 +114,52 @@ struct esc_bufset {
 
 namespace esc {
 
-struct Seg {                          // host-side flattened (row, segment) of a live<->slab pairing
-    uint8_t* live;
-    uint64_t slab_off;
-    uint64_t bytes;
+// Every verb runs on its context's device whatever the caller's current device is, and leaves the caller's current
+// device as it found it (include/esc.h "Devices").
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(const esc_ctx* c) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != c->device) {
+            err = cudaSetDevice(c->device);
+            switched = err == cudaSuccess;
+        }
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
 };
+#define ESC_ON_DEVICE(ctx)                 \
+    ::esc::DeviceGuard dev_guard__(ctx);   \
+    if (dev_guard__.err != cudaSuccess) return ::esc::cuda_fail(dev_guard__.err)
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize, once per (context, kernel instantiation `slot`); idempotent, so two threads
+// racing on the same slot only set it twice
+enum FuncSlot : uint32_t { kSlotGdn = 0, kSlotScan = 4 };   // scan instantiations take kSlotScan + their own index
+template <typename K>
+int ensure_dyn_smem(esc_ctx* ctx, uint32_t slot, K kernel, int bytes) {
+    const uint64_t bit = 1ull << slot;
+    if (ctx->func_attr_mask.load(std::memory_order_acquire) & bit) return ESC_OK;
+    ESC_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    ctx->func_attr_mask.fetch_or(bit, std::memory_order_release);
+    return ESC_OK;
+}
 
 uint64_t seg_valid(const Row& r, uint64_t P);
 int check_fit(const std::vector<Row>& rows, uint64_t P);
 // slab layout walk: fills segs (live pointers relative to `rows`), returns slab bytes / payload
 void layout_walk(const std::vector<Row>& rows, uint64_t P, std::vector<Seg>* segs, uint64_t* slab_bytes,
                  uint64_t* payload_bytes);
+// the same walk through the live set's one-entry cache (rebuilt only when P changes)
+const SegCache& live_segs(esc_bufset* live, uint64_t P);
+// one copy-kernel launch per kCopyMaxSeg segments: live -> slab (to_slab) or slab -> live
+int launch_copy_segs(const esc_ctx* ctx, const std::vector<Seg>& segs, uint8_t* slab, bool to_slab, cudaStream_t stream);
+// the restore node's table for (live segments, capsule slab)
+void build_restore_table(CopyTable* t, const std::vector<Seg>& segs, const uint8_t* slab);
 
 // copy kernel launchers (copy_kernel.cu)
 uint32_t copy_grid_blocks(uint64_t n_tiles);
@@ -131,10 +185,10 @@ struct ScanShape {
     uint32_t B, H, dk, dv, in_dtype, out_dtype, chunk;
 };
 bool decode_key(esc_shape_key key, ScanShape* s);
-int launch_scan(const esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g,
+int launch_scan(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g,
                 const float* state_in, float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream);
 // gated delta rule, chunked form on warp-level MMAs (gdn_mma_kernel.cu)
-int launch_gdn_mma(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* beta,
+int launch_gdn_mma(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* beta,
                    const float* state_in, float* state_out, float* o, uint64_t T, uint64_t t_stride, cudaStream_t stream);
 
 }  // namespace esc

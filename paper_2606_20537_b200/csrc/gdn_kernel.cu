@@ -143,7 +143,8 @@ int esc_gdn_scan(esc_ctx* ctx, esc_shape_key key, const void* q, const void* k, 
     if (s.out_dtype != ESC_DTYPE_F32) return ESC_ERR_UNSUPPORTED;
     const uintptr_t all = (uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)state_in | (uintptr_t)state_out | (uintptr_t)o;
     if ((all & 15u) || (((uintptr_t)g | (uintptr_t)beta) & 3u)) return ESC_ERR_UNALIGNED;
-    return launch_gdn_mma(s, q, k, v, g, beta, state_in, state_out, (float*)o, T, t_stride, (cudaStream_t)stream);
+    ESC_ON_DEVICE(ctx);
+    return launch_gdn_mma(ctx, s, q, k, v, g, beta, state_in, state_out, (float*)o, T, t_stride, (cudaStream_t)stream);
 }
 
 int esc_causal_conv(esc_ctx* ctx, const void* x, const float* w, const float* state_in, float* state_out, float* y, uint32_t B,
@@ -152,8 +153,9 @@ int esc_causal_conv(esc_ctx* ctx, const void* x, const float* w, const float* st
     if (T > 0 && (!x || !y)) return ESC_ERR_INVALID;
     if (W < 1 || W > (uint32_t)kConvMaxW || (C % 8) != 0) return ESC_ERR_UNSUPPORTED;
     if ((((uintptr_t)x | (uintptr_t)y) & 15u) || (((uintptr_t)w | (uintptr_t)state_in | (uintptr_t)state_out) & 3u)) return ESC_ERR_UNALIGNED;
+    if (T > 0 && B > 65535) return ESC_ERR_UNSUPPORTED;
+    ESC_ON_DEVICE(ctx);
     if (T > 0) {
-        if (B > 65535) return ESC_ERR_UNSUPPORTED;
         dim3 grid((C / kConvCPT + kConvThreads - 1) / kConvThreads, (uint32_t)((T + kConvRun - 1) / kConvRun), B);
         conv_kernel_for(W)<<<grid, kConvThreads, 0, (cudaStream_t)stream>>>((const __nv_bfloat16*)x, w, state_in, y, T, t_stride, C,
                                                                             flags & ESC_CONV_SILU);

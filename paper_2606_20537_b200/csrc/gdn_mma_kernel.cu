@@ -601,13 +601,10 @@ __global__ void __launch_bounds__(kGmThreads, 1) esc_gdn_mma_kernel(const __nv_b
 }
 
 template <int DK>
-static int launch_gdn_mma_t(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* beta,
+static int launch_gdn_mma_t(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* beta,
                             const float* state_in, float* state_out, float* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        ESC_CUDA(cudaFuncSetAttribute(esc_gdn_mma_kernel<DK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GmSmem<DK>)));
-        attr_set = true;
-    }
+    const int rc = ensure_dyn_smem(ctx, kSlotGdn + (DK == 128 ? 0 : 1), esc_gdn_mma_kernel<DK>, (int)sizeof(GmSmem<DK>));
+    if (rc != ESC_OK) return rc;
     dim3 grid(s.dv / kGmDVT, s.B * s.H);
     esc_gdn_mma_kernel<DK><<<grid, kGmThreads, sizeof(GmSmem<DK>), stream>>>(
         (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, g, beta, state_in, state_out, o, s.H, s.dv, T, t_stride);
@@ -619,11 +616,11 @@ static int launch_gdn_mma_t(const ScanShape& s, const void* q, const void* k, co
 extern "C" void esc_debug_gm_prof(long long* out24) { cudaMemcpyFromSymbol(out24, g_gm_prof, sizeof(g_gm_prof)); }
 #endif
 
-int launch_gdn_mma(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* beta,
+int launch_gdn_mma(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* beta,
                    const float* state_in, float* state_out, float* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
     if (s.dv % kGmDVT) return ESC_ERR_UNSUPPORTED;
-    if (s.dk == 128) return launch_gdn_mma_t<128>(s, q, k, v, g, beta, state_in, state_out, o, T, t_stride, stream);
-    if (s.dk == 64) return launch_gdn_mma_t<64>(s, q, k, v, g, beta, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 128) return launch_gdn_mma_t<128>(ctx, s, q, k, v, g, beta, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 64) return launch_gdn_mma_t<64>(ctx, s, q, k, v, g, beta, state_in, state_out, o, T, t_stride, stream);
     return ESC_ERR_UNSUPPORTED;
 }
 

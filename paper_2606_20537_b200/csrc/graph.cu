@@ -1,9 +1,12 @@
 // Captured replay plan: [restore node] -> [scan node per layer] as ONE CUDA graph
 // (include/esc.h: esc_graph_*).  PAPER.md:128-129: restore "replay[s] the already-captured
 // Graph[key] — never a recapture"; the host overwrites a bound sub-buffer between
-// replays.  Here the bound sub-buffer is the restore node's copy table: it lives in device
-// memory owned by the graph, so binding another capsule is one small async H2D copy and the
-// graph's kernel nodes (pointers, grids) never change.
+// replays.  Here the bound sub-buffer is the restore node's copy table: it lives in a small
+// caller-owned device scratch buffer (esc_graph_scratch_bytes), and binding another capsule is one
+// one-CTA kernel that stores the new table there (the table travels as a kernel parameter: no copy
+// engine, no host-side wait); the graph's kernel nodes (pointers, grids) never change.
+#include <string.h>
+
 #include <new>
 
 #include "esc_internal.h"
@@ -13,9 +16,11 @@ struct esc_graph {
     esc_bufset* live;             // NULL: cold plan (no restore node)
     cudaGraph_t graph;
     cudaGraphExec_t exec;
-    esc::CopyTable* table_dev;    // device-resident "current capsule" table (rewritten by a one-CTA kernel: launch_table_store)
+    esc::CopyTable* table_dev;    // device-resident "current capsule" table in the CALLER's scratch (rewritten by launch_table_store)
     bool bound;
+    bool owned_by_table;          // held by the context's Graph[key] table: only the table may destroy it
     uint64_t bound_boundary;
+    uint64_t max_boundary;        // the restore node's grid covers capsules up to this boundary
 };
 
 using namespace esc;
@@ -32,17 +37,24 @@ static void graph_free(esc_graph* g) {
     if (!g) return;
     if (g->exec) cudaGraphExecDestroy(g->exec);
     if (g->graph) cudaGraphDestroy(g->graph);
-    if (g->table_dev) cudaFree(g->table_dev);
-    delete g;
+    delete g;                     // the table lives in caller-owned scratch: nothing to free on the device
 }
 
 extern "C" {
 
+uint64_t esc_graph_scratch_bytes(void) { return sizeof(CopyTable); }
+
 int esc_graph_capture(esc_ctx* ctx, esc_bufset* live, uint64_t max_boundary, const esc_scan_args* layers,
-                      uint32_t n_layers, void* stream, esc_graph** out_graph) {
+                      uint32_t n_layers, void* scratch_dev, uint64_t scratch_bytes, void* stream, esc_graph** out_graph) {
     if (!ctx || !out_graph || (n_layers && !layers) || (!live && n_layers == 0)) return ESC_ERR_INVALID;
     if (!stream) return ESC_ERR_INVALID;  // the legacy default stream cannot be captured
-    if (live && live->frozen) return ESC_ERR_INVALID;
+    if (live && (live->frozen || live->ctx != ctx)) return ESC_ERR_INVALID;
+    if (live) {   // the restore node's table lives in the caller's scratch
+        if (!scratch_dev) return ESC_ERR_INVALID;
+        if ((uintptr_t)scratch_dev & 15u) return ESC_ERR_UNALIGNED;
+        if (scratch_bytes < sizeof(CopyTable)) return ESC_ERR_CAPACITY;
+    }
+    ESC_ON_DEVICE(ctx);
     uint32_t grid = 0;
     if (live) {
         int rc = check_fit(live->rows, max_boundary);
@@ -74,16 +86,23 @@ int esc_graph_capture(esc_ctx* ctx, esc_bufset* live, uint64_t max_boundary, con
     g->ctx = ctx;
     g->live = live;
     g->bound = false;
+    g->owned_by_table = false;
+    g->max_boundary = max_boundary;
     cudaError_t e = cudaSuccess;
+    cudaStream_t st = (cudaStream_t)stream;
     if (live) {
-        e = cudaMalloc((void**)&g->table_dev, sizeof(CopyTable));
-        if (e == cudaSuccess) e = cudaMemset(g->table_dev, 0, sizeof(CopyTable));  // n_tiles = 0: a no-op until bound
-        if (e != cudaSuccess) {
+        // an empty table (n_tiles = 0: the restore node is a no-op until a capsule is bound), stored by a kernel on the
+        // CALLER's stream ahead of the capture: ordered before every later launch / set_capsule on that stream, unlike a
+        // memset on the legacy stream, which a non-blocking stream does not wait for
+        g->table_dev = (CopyTable*)scratch_dev;
+        CopyTable empty;
+        memset(&empty, 0, sizeof empty);
+        int rc0 = launch_table_store(empty, g->table_dev, st);
+        if (rc0 != ESC_OK) {
             graph_free(g);
-            return cuda_fail(e);
+            return rc0;
         }
     }
-    cudaStream_t st = (cudaStream_t)stream;
     e = cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal);
     if (e != cudaSuccess) {
         graph_free(g);
@@ -114,21 +133,14 @@ int esc_graph_set_capsule(esc_graph* graph, const esc_bufset* capsule, void* str
     esc_bufset* live = graph->live;
     if (live->layout_digest != capsule->layout_digest || live->rows.size() != capsule->rows.size())
         return ESC_ERR_MISMATCH;
+    if (capsule->position > graph->max_boundary) return ESC_ERR_CAPACITY;   // the plan was sized for boundaries <= max_boundary
     int rc = check_fit(live->rows, capsule->position);
     if (rc != ESC_OK) return rc;
-    std::vector<Seg> segs;
-    layout_walk(live->rows, capsule->position, &segs, nullptr, nullptr);
+    ESC_ON_DEVICE(graph->ctx);
+    const std::vector<Seg>& segs = live_segs(live, capsule->position).segs;
     if (segs.size() > kCopyMaxSeg) return ESC_ERR_UNSUPPORTED;
-    std::vector<const uint8_t*> src(segs.size());
-    std::vector<uint8_t*> dst(segs.size());
-    std::vector<uint64_t> bytes(segs.size());
-    for (size_t i = 0; i < segs.size(); ++i) {
-        src[i] = capsule->slab + segs[i].slab_off;
-        dst[i] = segs[i].live;
-        bytes[i] = segs[i].bytes;
-    }
     CopyTable t;
-    build_copy_table(&t, src.data(), dst.data(), bytes.data(), (uint32_t)segs.size());
+    build_restore_table(&t, segs, capsule->slab);
     rc = launch_table_store(t, graph->table_dev, (cudaStream_t)stream);
     if (rc != ESC_OK) return rc;
     graph->bound = true;
@@ -139,6 +151,7 @@ int esc_graph_set_capsule(esc_graph* graph, const esc_bufset* capsule, void* str
 int esc_graph_launch(esc_graph* graph, void* stream) {
     if (!graph) return ESC_ERR_INVALID;
     if (graph->live && !graph->bound) return ESC_ERR_INVALID;
+    ESC_ON_DEVICE(graph->ctx);
     ESC_CUDA(cudaGraphLaunch(graph->exec, (cudaStream_t)stream));
     if (graph->live) {
         graph->live->position = graph->bound_boundary;
@@ -149,6 +162,8 @@ int esc_graph_launch(esc_graph* graph, void* stream) {
 
 int esc_graph_destroy(esc_graph* graph) {
     if (!graph) return ESC_ERR_INVALID;
+    if (graph->owned_by_table) return ESC_ERR_INVALID;   // the Graph[key] table owns it (evicts / destroys it itself)
+    ESC_ON_DEVICE(graph->ctx);
     graph_free(graph);
     return ESC_OK;
 }
@@ -173,6 +188,7 @@ uint64_t esc_plan_key_make(esc_shape_key key, uint64_t suffix_bucket, uint64_t m
 }
 
 static void plan_evict_to(esc_ctx* ctx, size_t n) {
+    DeviceGuard g(ctx);
     while (ctx->plans.size() > n) {
         graph_free(ctx->plans.back().second);
         ctx->plans.pop_back();
@@ -189,16 +205,31 @@ int esc_plan_table_set_capacity(esc_ctx* ctx, uint32_t capacity) {
 
 int esc_plan_table_put(esc_ctx* ctx, uint64_t plan_key, esc_graph* graph) {
     if (!ctx || !graph || graph->ctx != ctx) return ESC_ERR_INVALID;
-    for (size_t i = 0; i < ctx->plans.size(); ++i) {
-        if (ctx->plans[i].second == graph && ctx->plans[i].first != plan_key) return ESC_ERR_INVALID;   // already owned under another key
+    // a plan is owned once: the whole table is searched for the handle before anything changes
+    for (size_t i = 0; i < ctx->plans.size(); ++i)
+        if (ctx->plans[i].second == graph && ctx->plans[i].first != plan_key) return ESC_ERR_INVALID;
+    for (size_t i = 0; i < ctx->plans.size(); ++i)
         if (ctx->plans[i].first == plan_key) {
-            if (ctx->plans[i].second != graph) graph_free(ctx->plans[i].second);
+            if (ctx->plans[i].second != graph) {
+                DeviceGuard g(ctx);
+                graph_free(ctx->plans[i].second);
+            }
             ctx->plans.erase(ctx->plans.begin() + i);
             break;
         }
-    }
     plan_evict_to(ctx, ctx->plan_capacity - 1);
+    graph->owned_by_table = true;
     ctx->plans.insert(ctx->plans.begin(), std::make_pair(plan_key, graph));
+    return ESC_OK;
+}
+
+// 1 when `plan_key` is in the table (does not touch the LRU order or the statistics): lets a binding drop its references
+// to plans the table has evicted
+int esc_plan_table_contains(const esc_ctx* ctx, uint64_t plan_key, uint32_t* out_present) {
+    if (!ctx || !out_present) return ESC_ERR_INVALID;
+    *out_present = 0;
+    for (const auto& e : ctx->plans)
+        if (e.first == plan_key) *out_present = 1;
     return ESC_OK;
 }
 

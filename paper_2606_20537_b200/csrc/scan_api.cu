@@ -20,13 +20,12 @@ bool decode_key(esc_shape_key key, ScanShape* s) {
     return true;
 }
 
-int launch_scan_tc(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
+int launch_scan_tc(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                    float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream);
 
-int launch_scan(const esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g,
+int launch_scan(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g,
                 const float* state_in, float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
-    (void)ctx;
-    return launch_scan_tc(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    return launch_scan_tc(ctx, s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
 }
 
 }  // namespace esc
@@ -58,6 +57,7 @@ int esc_linattn_scan(esc_ctx* ctx, esc_shape_key key, const void* q, const void*
     const uintptr_t all = (uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)state_in | (uintptr_t)state_out |
                           (uintptr_t)o;
     if ((all & 15u) || ((uintptr_t)g & 3u)) return ESC_ERR_UNALIGNED;  // g is read element-wise: 4-B alignment
+    ESC_ON_DEVICE(ctx);
     return launch_scan(ctx, s, q, k, v, g, state_in, state_out, o, T, t_stride, (cudaStream_t)stream);
 }
 

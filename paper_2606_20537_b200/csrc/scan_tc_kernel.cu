@@ -795,13 +795,13 @@ static int make_tmap_halves(CUtensorMap* m, const void* base, uint32_t D, uint32
 }
 
 template <int DK, int C, int CS, typename OutT>
-static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
+static int launch_tc_t(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                        float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
     using L = TcCfg<DK, C, CS>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        ESC_CUDA(cudaFuncSetAttribute(esc_scan_tc_kernel<DK, C, CS, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::total));
-        attr_set = true;
+    constexpr uint32_t slot = kSlotScan + (DK == 128 ? 0 : 1) + 2 * (CS > 1 ? 1 : 0) + 4 * (sizeof(OutT) == 4 ? 0 : 1);
+    {
+        const int rc = ensure_dyn_smem(ctx, slot, esc_scan_tc_kernel<DK, C, CS, OutT>, (int)L::total);
+        if (rc != ESC_OK) return rc;
     }
     if (!state_out) return ESC_OK;   // prepare-only call (before a stream capture)
     CUtensorMap tq, tk, tv;
@@ -840,10 +840,10 @@ static int launch_tc_t(const ScanShape& s, const void* q, const void* k, const v
 }
 
 template <int DK, int C, int CS>
-static int launch_tc_o(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
+static int launch_tc_o(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                        float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
-    if (s.out_dtype == ESC_DTYPE_F32) return launch_tc_t<DK, C, CS, float>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
-    return launch_tc_t<DK, C, CS, bf16>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.out_dtype == ESC_DTYPE_F32) return launch_tc_t<DK, C, CS, float>(ctx, s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    return launch_tc_t<DK, C, CS, bf16>(ctx, s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
 }
 
 // Cluster size: 4.  A cluster of 8 (all d_v slices of a d_v = 128 head) would share twice as much, but B200 can keep only 15
@@ -862,16 +862,16 @@ constexpr int kTcCluster = 4;
 constexpr uint64_t kTcShortT = ESC_TC_SHORT;
 
 template <int DK, int C>
-static int launch_tc_dv(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
+static int launch_tc_dv(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                         float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
     if (s.dv % (kTcDVT * kTcCluster)) return ESC_ERR_UNSUPPORTED;
     if (!state_out) {   // prepare-only call: both variants
-        const int rc = launch_tc_o<DK, C, 1>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+        const int rc = launch_tc_o<DK, C, 1>(ctx, s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
         if (rc != ESC_OK) return rc;
     } else if (T <= kTcShortT) {
-        return launch_tc_o<DK, C, 1>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+        return launch_tc_o<DK, C, 1>(ctx, s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
     }
-    return launch_tc_o<DK, C, kTcCluster>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    return launch_tc_o<DK, C, kTcCluster>(ctx, s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
 }
 
 // The key's chunk (64 or 128) is the alignment grid the caller commits to (restore boundaries are multiples of it); the
@@ -879,11 +879,11 @@ static int launch_tc_dv(const ScanShape& s, const void* q, const void* k, const 
 // restore + continue stays bit-identical to the cold run), and the 64-token tile is 2.1x faster than a 128-token one
 // (r01 sweep: 83 M vs 38 M tokens/s at T = 64k — A grows quadratically with the tile and leaves no room for buffering).
 // The kernel template stays generic in C (the 128-token instantiation passed the same parity tests before this change).
-int launch_scan_tc(const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
+int launch_scan_tc(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* state_in,
                    float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
     if (s.chunk != 64 && s.chunk != 128) return ESC_ERR_UNSUPPORTED;
-    if (s.dk == 128) return launch_tc_dv<128, 64>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
-    if (s.dk == 64) return launch_tc_dv<64, 64>(s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 128) return launch_tc_dv<128, 64>(ctx, s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
+    if (s.dk == 64) return launch_tc_dv<64, 64>(ctx, s, q, k, v, g, state_in, state_out, o, T, t_stride, stream);
     return ESC_ERR_UNSUPPORTED;
 }
 

@@ -192,6 +192,7 @@ int esc_dequant_stage_fill(esc_bufset* live, uint32_t row, uint64_t upto_tokens,
         }
     }
     if (src.empty()) return ESC_OK;
+    ESC_ON_DEVICE(live->ctx);
     int rc = launch_stage(live->ctx, src.data(), d8.data(), d16.data(), bytes.data(), scale.data(), (uint32_t)src.size(),
                           (cudaStream_t)stream);
     if (rc == ESC_OK)

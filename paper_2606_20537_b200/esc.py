@@ -89,7 +89,8 @@ _sig = {
     "esc_linattn_scan": (C.c_int, [_P, C.c_uint64] + [_P] * 7 + [C.c_uint64, C.c_uint64, C.c_uint32, _P]),
     "esc_gdn_scan": (C.c_int, [_P, C.c_uint64] + [_P] * 8 + [C.c_uint64, C.c_uint64, _P]),
     "esc_causal_conv": (C.c_int, [_P] * 6 + [C.c_uint32, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _P]),
-    "esc_graph_capture": (C.c_int, [_P, _P, C.c_uint64, C.POINTER(ScanArgs), C.c_uint32, _P, C.POINTER(_P)]),
+    "esc_graph_scratch_bytes": (C.c_uint64, []),
+    "esc_graph_capture": (C.c_int, [_P, _P, C.c_uint64, C.POINTER(ScanArgs), C.c_uint32, _P, C.c_uint64, _P, C.POINTER(_P)]),
     "esc_graph_set_capsule": (C.c_int, [_P, _P, _P]),
     "esc_graph_launch": (C.c_int, [_P, _P]),
     "esc_graph_destroy": (C.c_int, [_P]),
@@ -98,6 +99,7 @@ _sig = {
     "esc_plan_table_set_capacity": (C.c_int, [_P, C.c_uint32]),
     "esc_plan_table_put": (C.c_int, [_P, C.c_uint64, _P]),
     "esc_plan_table_get": (C.c_int, [_P, C.c_uint64, C.POINTER(_P)]),
+    "esc_plan_table_contains": (C.c_int, [_P, C.c_uint64, C.POINTER(C.c_uint32)]),
     "esc_plan_table_stats": (C.c_int, [_P, C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64),
                                        C.POINTER(C.c_uint64)]),
 }
@@ -159,14 +161,31 @@ class Ctx:
         return n.value
 
     # Graph[key] table (bounded, LRU): the context owns the plans put into it
+    def _reconcile_plans(self):
+        """Drop the python wrappers of plans the C table no longer holds (LRU eviction, capacity shrink, replacement):
+        their handles are dead, and their buffers need not be kept alive any longer."""
+        plans = getattr(self, "_plans", {})
+        for key in list(plans):
+            present = C.c_uint32()
+            _check(lib.esc_plan_table_contains(self.h, key, C.byref(present)), "esc_plan_table_contains")
+            if not present.value:
+                g = plans.pop(key)
+                g.h = None          # launch() / set_capsule() on an evicted plan now fail in python instead of in C
+                g._keep = ()
+
     def plan_table_set_capacity(self, n):
         _check(lib.esc_plan_table_set_capacity(self.h, n), "esc_plan_table_set_capacity")
+        self._reconcile_plans()
 
     def plan_put(self, plan_key, graph):
         _check(lib.esc_plan_table_put(self.h, plan_key, graph.h), "esc_plan_table_put")
         graph.owned = False
         self._plans = getattr(self, "_plans", {})
+        old = self._plans.get(plan_key)
+        if old is not None and old is not graph:
+            old.h, old._keep = None, ()
         self._plans[plan_key] = graph   # keeps the python references (buffers) of the plan alive
+        self._reconcile_plans()
 
     def plan_get(self, plan_key):
         """The captured plan or None ("a new shape needing capture")."""
@@ -185,6 +204,9 @@ class Ctx:
 
     def close(self):
         if self.h:
+            for g in getattr(self, "_plans", {}).values():
+                g.h, g._keep = None, ()
+            self._plans = {}
             lib.esc_ctx_destroy(self.h)
             self.h = None
 
@@ -324,8 +346,10 @@ def causal_conv(ctx, x, w, state_in, state_out, y, B, T, t_stride, Cch, W, flags
 
 
 def scan_args(key, q, k, v, g, state_in, state_out, o, T, t_stride, chunk):
-    return ScanArgs(key, _ptr(q), _ptr(k), _ptr(v), _ptr(g), _ptr(state_in), _ptr(state_out), _ptr(o),
-                    T, t_stride, chunk, 0)
+    a = ScanArgs(key, _ptr(q), _ptr(k), _ptr(v), _ptr(g), _ptr(state_in), _ptr(state_out), _ptr(o),
+                 T, t_stride, chunk, 0)
+    a._keep = (q, k, v, g, state_in, state_out, o)   # the struct holds raw addresses: keep the tensors alive with it
+    return a
 
 
 def suffix_bucket(T, chunk):
@@ -342,22 +366,44 @@ class Graph:
         self._keep = keep
         self.owned = owned      # False once a context's plan table owns the handle
 
+    def _handle(self, where):
+        if not self.h:
+            raise EscError(ERR_INVALID, where + " (plan destroyed or evicted from the Graph[key] table)")
+        return self.h
+
     def set_capsule(self, capsule, stream=None):
-        _check(lib.esc_graph_set_capsule(self.h, capsule.h, _stream(stream)), "esc_graph_set_capsule")
+        _check(lib.esc_graph_set_capsule(self._handle("esc_graph_set_capsule"), capsule.h, _stream(stream)),
+               "esc_graph_set_capsule")
 
     def launch(self, stream=None):
-        _check(lib.esc_graph_launch(self.h, _stream(stream)), "esc_graph_launch")
+        _check(lib.esc_graph_launch(self._handle("esc_graph_launch"), _stream(stream)), "esc_graph_launch")
 
     def destroy(self):
         if self.h and self.owned:
             lib.esc_graph_destroy(self.h)
-        self.h = None
+        if self.owned:
+            self.h = None
+            self._keep = ()
 
 
-def graph_capture(ctx, live, max_boundary, layers, stream):
-    """layers: list of ScanArgs; live may be None (cold plan).  stream must be a non-default stream."""
+def graph_scratch_bytes():
+    return int(lib.esc_graph_scratch_bytes())
+
+
+def graph_capture(ctx, live, max_boundary, layers, stream, scratch=None):
+    """layers: list of ScanArgs; live may be None (cold plan).  stream must be a non-default stream.
+    scratch: caller-owned device memory (torch uint8 tensor) of graph_scratch_bytes() for the restore node's descriptor
+    table; allocated here with torch when omitted (the library itself never allocates device memory)."""
     arr = (ScanArgs * max(1, len(layers)))(*layers)
     h = _P()
+    nbytes = 0
+    if live is not None:
+        if scratch is None:
+            import torch
+            dev = stream.device if hasattr(stream, "device") else "cuda"
+            scratch = torch.empty(graph_scratch_bytes(), dtype=torch.uint8, device=dev)
+        nbytes = scratch.numel() * scratch.element_size() if hasattr(scratch, "numel") else graph_scratch_bytes()
     _check(lib.esc_graph_capture(ctx.h, live.h if live is not None else None, max_boundary, arr, len(layers),
-                                 _stream(stream), C.byref(h)), "esc_graph_capture")
-    return Graph(h, keep=(live, tuple(layers)))
+                                 _ptr(scratch) if live is not None else None, nbytes, _stream(stream), C.byref(h)),
+           "esc_graph_capture")
+    return Graph(h, keep=(live, tuple(layers), scratch))

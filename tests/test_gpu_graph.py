@@ -297,8 +297,14 @@ def test_plan_table_lru_and_padded_bucket(esc):
     ctx.plan_table_set_capacity(2)
     pk = [esc.plan_key_make(key, bucket, 0, n) for n in (1, 2, 3)]
     assert ctx.plan_get(pk[0]) is None                       # a new shape needing capture
-    ctx.plan_put(pk[0], capture(1))
-    ctx.plan_put(pk[1], capture(2))
+    g0, g1 = capture(1), capture(2)
+    ctx.plan_put(pk[0], g0)
+    ctx.plan_put(pk[1], g1)
+    # ownership: a plan the table holds cannot be destroyed by the caller, nor be put under a second key
+    assert esc.lib.esc_graph_destroy(g0.h) == esc.ERR_INVALID
+    with pytest.raises(esc.EscError) as e:
+        ctx.plan_put(pk[2], g0)
+    assert e.value.code == esc.ERR_INVALID
     plan = ctx.plan_get(pk[0])                               # hit; pk[0] becomes most recently used
     assert plan is not None
     plan.launch(stream)
@@ -306,9 +312,49 @@ def test_plan_table_lru_and_padded_bucket(esc):
     assert bits_equal(o[:, :T], o_ref) and bits_equal(state, s_ref)
     ctx.plan_put(pk[2], capture(3))                          # table full: evicts the least recently used = pk[1]
     assert ctx.plan_get(pk[1]) is None and ctx.plan_get(pk[0]) is not None and ctx.plan_get(pk[2]) is not None
+    with pytest.raises(esc.EscError):                        # the evicted plan's wrapper is dead, not dangling
+        g1.launch(stream)
     st = ctx.plan_stats()
     assert st == {"size": 2, "hits": 3, "misses": 2, "evictions": 1}
     ctx.plan_table_set_capacity(1)                           # shrinking evicts down to the most recently used (pk[2])
     assert ctx.plan_get(pk[0]) is None and ctx.plan_get(pk[2]) is not None
     assert ctx.plan_stats()["evictions"] == 2
     ctx.close()                                              # the context destroys the plans it still owns
+
+
+def test_graph_scratch_and_capacity_contract(esc, ctx):
+    # include/esc.h "Ownership": the restore node's descriptor table lives in CALLER-owned scratch; a capsule later than the
+    # plan's max_boundary is refused; every error is reported before anything is enqueued.
+    specs = synth.hybrid_layout(256, n_linear=2, n_full=1, H=2, dk=64, dv=64, kv_heads=1, head_dim=64)
+    live = LiveSet(esc, ctx, specs, (90, 0))
+    stream = torch.cuda.Stream()
+    need = esc.graph_scratch_bytes()
+    assert 0 < need <= 8192
+
+    def raw_capture(scratch_ptr, nbytes):
+        h = esc._P()
+        arr = (esc.ScanArgs * 1)()
+        return esc.lib.esc_graph_capture(ctx.h, live.set.h, 128, arr, 0, scratch_ptr, nbytes, stream.cuda_stream, esc.C.byref(h))
+
+    big = torch.zeros(need + 64, dtype=torch.uint8, device=DEV)
+    assert raw_capture(None, 0) == esc.ERR_INVALID
+    assert raw_capture(big.data_ptr(), need - 1) == esc.ERR_CAPACITY
+    assert raw_capture(big.data_ptr() + 4, need) == esc.ERR_UNALIGNED
+    scratch = torch.full((need,), 0xAB, dtype=torch.uint8, device=DEV)    # garbage in the scratch must not matter
+    graph = esc.graph_capture(ctx, live.set, 128, [], stream, scratch=scratch)
+    slab = torch.empty(live.set.capsule_bytes(192)[0], dtype=torch.uint8, device=DEV)
+    cap_late = esc.snapshot(live.set, 192, 64, slab, stream=stream)
+    with pytest.raises(esc.EscError) as e:
+        graph.set_capsule(cap_late, stream)                  # boundary 192 > max_boundary 128
+    assert e.value.code == esc.ERR_CAPACITY
+    cap = esc.snapshot(live.set, 128, 64, slab, stream=stream)
+    stream.synchronize()
+    ref = oracle.capsule_snapshot(live.oracle_rows(), 128)
+    live.fill(91, 0, pattern=0xFF)
+    torch.cuda.synchronize()
+    graph.set_capsule(cap, stream)
+    graph.launch(stream)
+    stream.synchronize()
+    oracle.capsule_restore(live.oracle_rows(), 128, ref)
+    live.assert_equals_host()
+    graph.destroy()
