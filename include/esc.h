@@ -251,6 +251,11 @@ int esc_restore_ex(esc_bufset* live, const esc_bufset* capsule, const uint64_t* 
 esc_shape_key esc_shape_key_make(uint32_t B, uint32_t H, uint32_t d_k, uint32_t d_v,
                                  uint32_t in_dtype, uint32_t out_dtype, uint32_t chunk);
 
+/* The d_v tile of the scan kernel for `key` on the context's device (16 or 32 columns per CTA).  It is a function of the
+ * key and the device only — T never enters — which is what lets a cold run and a restore-then-continue run of one key share
+ * their arithmetic bit for bit.  Informational: the tests assert the property through it. */
+int esc_scan_tile_columns(const esc_ctx* ctx, esc_shape_key key, uint32_t* out_columns);
+
 /*
  * linattn_scan: for every (b,h), with S_0 = state_in[b,h],
  *      S_t = g_t * S_{t-1} + k_t^T v_t ,   o_t = q_t S_t ,   state_out[b,h] = S_T

@@ -185,6 +185,8 @@ struct ScanShape {
     uint32_t B, H, dk, dv, in_dtype, out_dtype, chunk;
 };
 bool decode_key(esc_shape_key key, ScanShape* s);
+// d_v columns per CTA of the scan kernel: a function of the shape key (and the device's SM count) only, never of T
+uint32_t scan_tile_columns(const esc_ctx* ctx, const ScanShape& s);
 int launch_scan(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g,
                 const float* state_in, float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream);
 // gated delta rule, chunked form on warp-level MMAs (gdn_mma_kernel.cu)

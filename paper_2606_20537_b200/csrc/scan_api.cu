@@ -1,5 +1,5 @@
 // Host side of esc_linattn_scan (include/esc.h): shape key, argument checks, dispatch to the sm_100a
-// tensor-core kernel in scan_tc_kernel.cu.  There is one scan kernel and no fallback.
+// tensor-core kernel in scan_kernel.cu.  There is one scan kernel and no fallback.
 #include "esc_internal.h"
 
 namespace esc {
@@ -43,6 +43,13 @@ esc_shape_key esc_shape_key_make(uint32_t B, uint32_t H, uint32_t d_k, uint32_t 
     if (!(out_dtype == ESC_DTYPE_F32 || out_dtype == ESC_DTYPE_BF16)) return 0;
     return (kKeyTag << 56) | ((uint64_t)B << 40) | ((uint64_t)H << 28) | ((uint64_t)(d_k / 8) << 20) |
            ((uint64_t)(d_v / 8) << 12) | ((uint64_t)in_dtype << 10) | ((uint64_t)out_dtype << 8) | (uint64_t)(chunk / 8);
+}
+
+int esc_scan_tile_columns(const esc_ctx* ctx, esc_shape_key key, uint32_t* out_columns) {
+    ScanShape s;
+    if (!ctx || !out_columns || !decode_key(key, &s)) return ESC_ERR_INVALID;
+    *out_columns = scan_tile_columns(ctx, s);
+    return ESC_OK;
 }
 
 int esc_linattn_scan(esc_ctx* ctx, esc_shape_key key, const void* q, const void* k, const void* v, const float* g,

@@ -195,6 +195,15 @@ __device__ __forceinline__ void tmem_ld_16x256b_x8(uint32_t addr, uint32_t* r) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// registers -> TMEM.  16 lanes x 128 bit (4 columns) per matrix, x2 = 8 columns: thread t writes rows {t/4, t/4+8} of the 16
+// lanes; per 4-column matrix m: r[2m] -> (row t/4, column 4m + t%4), r[2m+1] -> (row t/4+8, same column)
+// (layout confirmed on B200 by a store / 32x32b-load round trip, r02)
+__device__ __forceinline__ void tmem_st_16x128b_x2(uint32_t addr, const uint32_t* r) {
+    asm volatile("tcgen05.st.sync.aligned.16x128b.x2.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3])
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
 // ---- tcgen05.mma -------------------------------------------------------------------------------
 // D[tmem] (+)= A[smem] * B[smem], bf16 x bf16 -> fp32; issued by ONE thread
 __device__ __forceinline__ void mma_bf16_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, bool accumulate) {
@@ -203,6 +212,16 @@ __device__ __forceinline__ void mma_bf16_ss(uint32_t d_tmem, uint64_t a_desc, ui
         "setp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
         ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"((uint32_t)accumulate)
+        : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem]: the A operand (M rows in the accumulator's lane layout, bf16 pairs packed two per 32-bit
+// column, K-major) is read from tensor memory
+__device__ __forceinline__ void mma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, bool accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"((uint32_t)accumulate)
         : "memory");
 }
 // arrive on an mbarrier when every tcgen05.mma issued so far by this thread has completed

@@ -86,6 +86,7 @@ _sig = {
     "esc_restore_ex": (C.c_int, [_P, _P, C.POINTER(C.c_uint64), C.c_uint32, _P]),
     "esc_capsule_valid_end": (C.c_int, [_P, C.c_uint32, C.POINTER(C.c_uint64)]),
     "esc_shape_key_make": (C.c_uint64, [C.c_uint32] * 7),
+    "esc_scan_tile_columns": (C.c_int, [_P, C.c_uint64, C.POINTER(C.c_uint32)]),
     "esc_linattn_scan": (C.c_int, [_P, C.c_uint64] + [_P] * 7 + [C.c_uint64, C.c_uint64, C.c_uint32, _P]),
     "esc_gdn_scan": (C.c_int, [_P, C.c_uint64] + [_P] * 8 + [C.c_uint64, C.c_uint64, _P]),
     "esc_causal_conv": (C.c_int, [_P] * 6 + [C.c_uint32, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _P]),
@@ -328,6 +329,12 @@ def capsule_promote(host_capsule, storage_dev, storage_bytes=None, stream=None):
 
 def rollback(live, capsule_earlier, stream=None):
     _check(lib.esc_rollback(live.h, capsule_earlier.h, _stream(stream)), "esc_rollback")
+
+
+def scan_tile_columns(ctx, key):
+    w = C.c_uint32()
+    _check(lib.esc_scan_tile_columns(ctx.h, key, C.byref(w)), "esc_scan_tile_columns")
+    return w.value
 
 
 def linattn_scan(ctx, key, q, k, v, g, state_in, state_out, o, T, t_stride, chunk, stream=None):
