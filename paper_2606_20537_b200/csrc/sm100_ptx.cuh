@@ -22,8 +22,20 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+#ifndef ESC_MBAR_SUSPEND_NS
+#define ESC_MBAR_SUSPEND_NS 0
+#endif
 __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
     uint32_t ok;
+#if ESC_MBAR_SUSPEND_NS > 0
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity), "r"((uint32_t)ESC_MBAR_SUSPEND_NS)
+        : "memory");
+#else
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
@@ -31,11 +43,22 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
         : "=r"(ok)
         : "r"(smem_u32(bar)), "r"(parity)
         : "memory");
+#endif
     return ok != 0;
 }
 // (a suspend-time hint or a nanosleep back-off in this loop changed nothing measurable: r01 experiments)
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) {
+    }
+}
+
+// the same with a chosen back-off between polls.  A failed try_wait returns after a few tens of cycles, and every retry costs
+// three issue slots; with ~25 warps per CTA, most of them waiting most of the time, a third of all issued instructions were
+// retries (r02 ncu source page: 620 polls per chunk and CTA) in a kernel whose schedulers issue 73 % of the cycles.
+template <uint32_t kNs>
+__device__ __forceinline__ void mbar_wait_ns(uint64_t* bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {
+        if (kNs) asm volatile("nanosleep.u32 %0;" ::"r"(kNs));
     }
 }
 

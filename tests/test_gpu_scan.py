@@ -56,6 +56,13 @@ SHAPES = [
     (1, 1, 128, 128, 63, 64, "fast"),       # T < chunk
     (2, 3, 64, 64, 128, 64, "fast"),        # two whole chunks in the cluster-free short-call variant (T <= 128), d = 64
     (1, 2, 128, 64, 100, 128, "slow"),      # ragged second chunk in the short-call variant, d_v = 64
+    # the 32-column tile (B H d_v / 16 > SMs): every (d_k, cluster size) instantiation, long and short calls
+    (2, 16, 128, 128, 330, 64, "slow"),     # d_k 128, clusters of 4
+    (2, 16, 128, 128, 100, 64, "fast"),     #   ... cluster-free short call
+    (2, 10, 64, 128, 300, 64, "slow"),      # d_k 64, clusters of 4
+    (2, 20, 128, 64, 333, 128, "fast"),     # d_v 64: clusters of 2
+    (2, 20, 64, 64, 200, 64, "slow"),       # d_k 64, d_v 64: clusters of 2
+    (2, 20, 64, 64, 64, 64, "one"),         #   ... cluster-free short call
 ]
 
 
@@ -102,6 +109,9 @@ def test_batch_stride_and_untouched_tail(esc, ctx):
     (1, 2, 64, 64, 256, 64, 128),          # config 0: snapshot at t=128, restore, continue 128
     (2, 4, 128, 128, 448, 64, 192),
     (1, 4, 128, 128, 640, 128, 384),
+    (2, 16, 128, 128, 448, 64, 192),       # 32-column tile, long continuation (clusters of 4)
+    (4, 16, 128, 128, 320, 64, 256),       # 32-column tile, continuation of 64 tokens: the cluster-free launch
+    (2, 20, 64, 64, 384, 128, 256),        # d = 64, clusters of 2
 ])
 def test_aligned_restore_continue_is_bit_identical_to_cold(esc, ctx, B, H, dk, dv, T, chunk, P):
     si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(13, T, P))
@@ -230,10 +240,12 @@ def test_config4_sweep_points_sampled(esc, ctx, B, T, chunk):
     _check_sampled_heads(si, o_m, s_tm, pairs[:1], t_from=Pm)   # misaligned restore: oracle tolerance only
 
 
-def test_back_to_back_scans_on_one_stream_are_ordered(esc, ctx):
+@pytest.mark.parametrize("B", [1, 2, 4])
+def test_back_to_back_scans_on_one_stream_are_ordered(esc, ctx, B):
     # the scan kernel allows programmatic dependent launch: a following scan may start its on-chip setup early but must
-    # not read the state the previous one is still writing.  20 chained in-place suffix scans == one scan over all tokens.
-    B, H, dk, dv, chunk, n, T = 1, 16, 128, 128, 64, 20, 20 * 64
+    # not read the state the previous one is still writing.  20 chained in-place suffix scans == one scan over all tokens
+    # (B = 1: the 16-column tile; B = 2, 4: the 32-column tile).
+    H, dk, dv, chunk, n, T = 16, 128, 128, 64, 20, 20 * 64
     si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(18,), gate="slow")
     dev_in = scan_dev_inputs(si)
     o_cold, s_cold, _ = run_scan(esc, ctx, dev_in, B, T, H, dk, dv, chunk)
@@ -254,21 +266,39 @@ def test_back_to_back_scans_on_one_stream_are_ordered(esc, ctx):
         assert bits_equal(o, o_cold) and bits_equal(state, s_cold)
 
 
-def test_short_call_variant_matches_long_call_prefix_bitwise(esc, ctx):
-    # calls of up to 128 tokens run the kernel without a cluster (every CTA computes all score columns itself); longer ones
-    # in clusters of 4 that exchange score slices.  Causality makes o[:, :T] of a long call a function of the first T tokens
-    # only, so it must equal the short call's o bit for bit, ragged T included; so must the carried state at chunk multiples.
-    B, H, dk, dv, chunk, T_long = 2, 16, 128, 128, 64, 448
-    si = synth.scan_inputs(B, T_long, H, dk, dv, seed_ids=(21,), gate="slow")
+def test_tile_is_a_function_of_the_key_not_of_T(esc, ctx):
+    # DESIGN.md reading 11 / 26: the d_v tile is chosen from (B, H, d_v) and the device only; the call never sees T
+    k1 = esc.shape_key_make(1, 16, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, 64)
+    k2 = esc.shape_key_make(2, 16, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, 64)
+    k4 = esc.shape_key_make(4, 16, 128, 128, esc.DTYPE_BF16, esc.DTYPE_BF16, 128)
+    ks = esc.shape_key_make(1, 2, 64, 64, esc.DTYPE_BF16, esc.DTYPE_F32, 64)
+    assert esc.scan_tile_columns(ctx, k1) == 16 and esc.scan_tile_columns(ctx, ks) == 16     # one wave of 16-column CTAs
+    assert esc.scan_tile_columns(ctx, k2) == 32 and esc.scan_tile_columns(ctx, k4) == 32
+
+
+@pytest.mark.parametrize("B,H,dk,dv,out_bf16", [
+    (2, 16, 128, 128, False),    # 32-column tile (the historical case)
+    (1, 16, 128, 128, False),    # 16-column tile
+    (4, 16, 128, 128, True),     # 32-column tile, bf16 o
+    (2, 20, 64, 64, False),      # d = 64, 32-column tile, clusters of 2
+    (1, 4, 64, 64, True),        # d = 64, 16-column tile, bf16 o
+])
+def test_short_call_variant_matches_long_call_prefix_bitwise(esc, ctx, B, H, dk, dv, out_bf16):
+    # calls of up to 128 tokens launch the kernel without its cluster (whole-tile TMA loads instead of multicast row slices);
+    # the arithmetic is the same.  Causality makes o[:, :T] of a long call a function of the first T tokens only, so it must
+    # equal the short call's o bit for bit, ragged T included; so must the carried state at chunk multiples.  Every d_v tile,
+    # d = 64 and the bf16-o variant are covered (the proof is by test, reading 26).
+    chunk, T_long = 64, 448
+    si = synth.scan_inputs(B, T_long, H, dk, dv, seed_ids=(21, B, H, dk), gate="slow")
     s0 = synth.scan_state(B, H, dk, dv, seed_ids=(21,), scale=0.3)
     dev_in = scan_dev_inputs(si)
     s0_dev = torch.from_numpy(s0).to(DEV)
-    o_long, _, _ = run_scan(esc, ctx, dev_in, B, T_long, H, dk, dv, chunk, s0=s0_dev)
+    o_long, _, _ = run_scan(esc, ctx, dev_in, B, T_long, H, dk, dv, chunk, s0=s0_dev, out_bf16=out_bf16)
     for T in (1, 37, 64, 100, 128):
-        o_short, s_short, _ = run_scan(esc, ctx, dev_in, B, T_long, H, dk, dv, chunk, s0=s0_dev, n=T)
+        o_short, s_short, _ = run_scan(esc, ctx, dev_in, B, T_long, H, dk, dv, chunk, s0=s0_dev, n=T, out_bf16=out_bf16)
         assert bits_equal(o_short[:, :T], o_long[:, :T]), T
         if T % chunk == 0:   # continue the long way from the short call's state: the rest of the long run, bit for bit
-            o_rest, _, _ = run_scan(esc, ctx, dev_in, B, T_long, H, dk, dv, chunk, s0=s_short, t0=T)
+            o_rest, _, _ = run_scan(esc, ctx, dev_in, B, T_long, H, dk, dv, chunk, s0=s_short, t0=T, out_bf16=out_bf16)
             assert bits_equal(o_rest, o_long[:, T:]), T
 
 
