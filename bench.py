@@ -39,7 +39,7 @@ def parse_args():
     ap.add_argument("--impl", default="esc", choices=["esc", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the scan / warm-vs-cold / cpu_baseline extras")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--profile", default=None, choices=["scan", "restore", "suffix", "gdn", "conv", "stage"],
+    ap.add_argument("--profile", default=None, choices=["scan", "scan32", "restore", "suffix", "gdn", "conv", "stage"],
                     help="ncu driver: launch only the cold 16448-token scan (x3), only the 66 MiB restore (x5) or only the 18 "
                          "64-token suffix scans (x2); no JSON line")
     return ap.parse_args()
@@ -818,6 +818,19 @@ def run_profile(args):
         key = esc.shape_key_make(1, 16, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
         for _ in range(3):
             esc.linattn_scan(ctx, key, *full.dev[0], None, sess.states[0], full.out[0], T, T, CHUNK, stream=stream)
+    elif args.profile == "scan32":     # the 32-column tile: BASELINE config 4's B = 4 point at T = 8192
+        Bp, T = 4, 8192
+        gen = torch.Generator(device="cuda:0")
+        gen.manual_seed(20537)
+        sq = torch.nn.functional.normalize(torch.randn((Bp, T, 16, 128), device="cuda:0", generator=gen), dim=-1).to(torch.bfloat16)
+        sk = torch.nn.functional.normalize(torch.randn((Bp, T, 16, 128), device="cuda:0", generator=gen), dim=-1).to(torch.bfloat16)
+        sv = torch.randn((Bp, T, 16, 128), device="cuda:0", generator=gen).to(torch.bfloat16)
+        sg = torch.sigmoid(-torch.randn((Bp, T, 16), device="cuda:0", generator=gen)).clamp_min(1e-30)
+        so = torch.empty((Bp, T, 16, 128), dtype=torch.float32, device="cuda:0")
+        ss = torch.empty((Bp, 16, 128, 128), dtype=torch.float32, device="cuda:0")
+        key = esc.shape_key_make(Bp, 16, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
+        for _ in range(3):
+            esc.linattn_scan(ctx, key, sq, sk, sv, sg, None, ss, so, T, T, CHUNK, stream=stream)
     elif args.profile == "gdn":
         from paper_2606_20537_b200 import synth
         T = 16384 + SUFFIX
