@@ -382,6 +382,13 @@ def run_esc(args):
     n_launch = launches[0]
     ms_step = sum(ms) / len(ms)
     step_stats = timing_stats(ms)
+    # host time of the step's C-ABI calls alone (snapshot + set_capsule + graph launch through the binding, no torch calls)
+    stream.synchronize()
+    h0 = time.perf_counter()
+    for i in range(50):
+        step(i)
+    host_api_us = (time.perf_counter() - h0) / 50 * 1e6
+    stream.synchronize()
 
     # ---- end to end: suffix inputs H2D from pinned memory + outputs D2H inside the timed region -------
     def step_e2e(i):
@@ -546,14 +553,16 @@ def run_esc(args):
     sfx_us = ms_suffix * 1e3 / N_LINEAR
     sfx_gbs = sfx_alg / (sfx_us * 1e-6) / 1e9
     tr, tr_note = measured_traffic("esc_scan_kernel_suffix")
-    roof_sfx = {"kernel": "esc scan kernel, short-call instantiation (B1 H16 d128, T=64 suffix: one chunk per (b,h); 18 launches per step)",
+    w_sfx = esc.scan_tile_columns(ctx, key)
+    roof_sfx = {"kernel": "esc_scan_kernel<128,%d,1,float> (B1 H16 d128, T=64 suffix: one chunk per (b,h), %d-column d_v tile, cluster-free "
+                          "launch; 18 launches per step)" % (w_sfx, w_sfx),
                 "bound": "hbm", "achieved": sfx_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": sfx_gbs / pk["hbm_gbs"],
                 "peak_source": pk["source"], "traffic": tr, "us_per_launch": sfx_us, "alg_bytes_per_launch": sfx_alg,
                 "traffic_note": tr_note,
                 "share_of_step": ms_suffix / ms_step,
                 "note": "latency-bound by construction: 3.4 MB per launch is 0.5 us of HBM time; the launch is one chunk of "
-                        "the dependent pipeline (TMA -> P -> scores -> O2 -> store) plus setup/teardown; calls of <= 128 tokens run the "
-                        "kernel without a cluster"}
+                        "the dependent pipeline (TMA -> [P|O1] -> scores -> O2 -> store) plus setup/teardown; calls of <= 128 tokens "
+                        "launch the kernel without its cluster"}
     dominant = roof_sfx if ms_suffix > ms_restore + ms_snapshot else roof_copy
     out = {
         "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -568,6 +577,10 @@ def run_esc(args):
         "clocks": clocks, "gpu_launches": n_launch, "wall_ms_timed_region": wall_ms,
         "e2e": {"value": e2e_value, "unit": "GB/s", "h2d_bytes_per_step": inputs.h2d_bytes(),
                 "d2h_bytes_per_step": inputs.d2h_bytes(), "ms_per_step": ms_e2e, "host_enqueue_ms_per_step": host_ms[0],
+                "host_enqueue_note": "host time to enqueue one pipelined step, torch stream / event / copy_ calls of the harness "
+                                     "included; the step's three C-ABI calls alone (snapshot, set_capsule, graph launch through "
+                                     "ctypes): %.1f us" % host_api_us,
+                "host_api_us_per_step": host_api_us,
                 "mode": "K steps back to back, double-buffered: H2D of step i+1 and D2H of step i-1 overlap step i "
                         "(separate streams); every step uploads its inputs from pinned memory and downloads its outputs",
                 "serial_ms_per_step": ms_e2e_serial, "serial_value": aggregate_value(moved, ms_e2e_serial, world),
@@ -656,7 +669,8 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
             flops = T * workload.H * (2 * CHUNK * (128 + 128) + 4 * 128 * 128)
             res["scan"] = {"tokens": T, "layers": 1, "ms": one_ms, "tokens_per_s": T / (one_ms * 1e-3),
                            "tokens_per_s_18_layer_cold_graph": T / (cold_ms * 1e-3), "alg_TFLOPs": flops / (one_ms * 1e-3) / 1e12}
-            res["roofline_scan_cold"] = {"kernel": "esc scan kernel, long-call instantiation (B1 H16 d128 T=16448 chunk 64: BASELINE config 2 cold scan, one layer)", "bound": "hbm",
+            res["roofline_scan_cold"] = {"kernel": "esc_scan_kernel<128,%d,4,float> (B1 H16 d128 T=16448 chunk 64: BASELINE config 2 cold scan, one layer, "
+                                                   "%d-column d_v tile, clusters of 4)" % (esc.scan_tile_columns(ctx, key), esc.scan_tile_columns(ctx, key)), "bound": "hbm",
                                     "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": gbs / pk["hbm_gbs"],
                                     "peak_source": pk["source"], "traffic": measured_traffic("esc_scan_kernel_cold")[0],
                                     "us_per_launch": one_ms * 1e3, "traffic_note": measured_traffic("esc_scan_kernel_cold")[1],
@@ -783,8 +797,8 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
     sweep = []
     gen = torch.Generator(device=dev)
     gen.manual_seed(20537)
-    for (Bs, Ts, Cs) in ((1, 2048, 64), (1, 8192, 64), (1, 32768, 64), (1, 65536, 64), (4, 8192, 64), (4, 32768, 64), (1, 8192, 128),
-                         (1, 65536, 128), (4, 32768, 128)):
+    for (Bs, Ts, Cs) in ((1, 2048, 64), (1, 8192, 64), (1, 32768, 64), (1, 65536, 64), (2, 32768, 64), (4, 8192, 64), (4, 32768, 64),
+                         (1, 8192, 128), (1, 65536, 128), (4, 32768, 128)):
         sq = torch.nn.functional.normalize(torch.randn((Bs, Ts, workload.H, 128), device=dev, generator=gen), dim=-1).to(torch.bfloat16)
         sk = torch.nn.functional.normalize(torch.randn((Bs, Ts, workload.H, 128), device=dev, generator=gen), dim=-1).to(torch.bfloat16)
         sv = torch.randn((Bs, Ts, workload.H, 128), device=dev, generator=gen).to(torch.bfloat16)
@@ -794,7 +808,8 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
         skey = esc.shape_key_make(Bs, workload.H, 128, 128, esc.DTYPE_BF16, esc.DTYPE_F32, Cs)
         ms_, _ = med_ms(lambda: esc.linattn_scan(ctx, skey, sq, sk, sv, sg, None, ss, so, Ts, Ts, Cs, stream=stream), n=5, warm=1)
         alg_ = Bs * Ts * workload.H * ALG_BYTES_PER_TOKEN_HEAD + 2 * Bs * workload.H * 128 * 128 * 4
-        sweep.append({"B": Bs, "T": Ts, "chunk": Cs, "ms": ms_, "tokens_per_s": Bs * Ts / (ms_ * 1e-3),
+        sweep.append({"B": Bs, "T": Ts, "chunk": Cs, "tile_columns": esc.scan_tile_columns(ctx, skey), "ms": ms_,
+                      "tokens_per_s": Bs * Ts / (ms_ * 1e-3),
                       "frac_of_hbm_roofline": alg_ / (ms_ * 1e-3) / 1e9 / pk["hbm_gbs"]})
         del sq, sk, sv, sg, so, ss
         torch.cuda.empty_cache()
