@@ -277,7 +277,7 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
                 const int t0 = (int)(c * kC);
                 uint8_t* st = sm + L::stage_off + s * L::stage_bytes;
                 // the stage is free once the [P|O1] and U issuers of all CS CTAs have committed chunk c - NS
-                PW(0, mbar_wait_relaxed(&bars[BI.empty + s], ((c / NS) & 1) ^ 1));
+                if (CS > 1 || c >= (uint32_t)NS) PW(0, mbar_wait_relaxed(&bars[BI.empty + s], ((c / NS) & 1) ^ 1));   // (a short call's first round: fresh)
                 uint64_t* full = &bars[BI.full + s];
                 mbar_arrive_expect_tx(full, L::q_bytes + L::k_tile_bytes);   // arrives in CS row slices, one from each CTA
                 if constexpr (CS > 1) {
@@ -297,8 +297,10 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
                 }
                 // V tiles have a ring of their own: O2 (the end of the score path) reads V from it, so a Q/K stage is
                 // released as soon as [P|O1] and U are done with it
-                PW(1, mbar_wait_relaxed(&bars[BI.v_read + vi], ((c / NV) & 1) ^ 1));      // the V~ warps and O2 of chunk c - NV
-                PW(1, mbar_wait_relaxed(&bars[BI.o2_done + vi], ((c / NV) & 1) ^ 1));     // are done with V tile vi
+                if (CS > 1 || c >= (uint32_t)NV) {
+                    PW(1, mbar_wait_relaxed(&bars[BI.v_read + vi], ((c / NV) & 1) ^ 1));      // the V~ warps and O2 of chunk c - NV
+                    PW(1, mbar_wait_relaxed(&bars[BI.o2_done + vi], ((c / NV) & 1) ^ 1));     // are done with V tile vi
+                }
                 mbar_arrive_expect_tx(&bars[BI.v_full + vi], L::v_bytes);
                 tma_load_4d(sm + L::v_off + vi * L::v_bytes, &tv, &bars[BI.v_full + vi], (int)dv0, (int)h, t0, (int)b);
                 TC_TRACE(0, c);
@@ -337,7 +339,7 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
             const float prev = __shfl_up_sync(0xffffffffu, incl, 1);
             const float excl = (lane % GL) ? prev : 0.f;
             const uint32_t slot = bt & 1;
-            PW(0, mbar_wait_relaxed(&bars[BI.g_empty + slot], ((bt >> 1) & 1) ^ 1));
+            if (CS > 1 || bt >= 2) PW(0, mbar_wait_relaxed(&bars[BI.g_empty + slot], ((bt >> 1) & 1) ^ 1));
             float* b2 = gate + slot * 2 * kGateBatch;
             float* eb = b2 + kGateBatch;
 #pragma unroll
@@ -360,7 +362,7 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
             PW(0, mbar_wait(&bars[BI.full + s], (c / NS) & 1));
             // accumulator pb is free once the epilogue has read O1(c - NB) and O2(c - NB) has read A.  The O2 issuer is never
             // ahead of this warp, so the ring entry of chunk c - NB cannot have moved on to a later phase.
-            PW(1, mbar_wait(&bars[BI.po_read + pb], ((c / NB) & 1) ^ 1));
+            if (CS > 1 || c >= (uint32_t)NB) PW(1, mbar_wait(&bars[BI.po_read + pb], ((c / NB) & 1) ^ 1));
             if (c >= (uint32_t)NB) PW(1, mbar_wait(&bars[BI.o2_done + (c - NB) % NV], ((c - NB) / NV) & 1));
             PW(2, mbar_wait(&bars[BI.s_full + s], (c / NS) & 1));      // the carried state: last, it is the one on the chain
             tc_fence_after_sync();
@@ -382,7 +384,7 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
         for (uint32_t c = 0; c < n_chunks; ++c) {
             const uint32_t s = c % NS, vb = c % NVT, ob = c % NUB;
             PW(0, mbar_wait(&bars[BI.full + s], (c / NS) & 1));
-            PW(1, mbar_wait(&bars[BI.u_empty + ob], ((c / NUB) & 1) ^ 1));
+            if (CS > 1 || c >= (uint32_t)NUB) PW(1, mbar_wait(&bars[BI.u_empty + ob], ((c / NUB) & 1) ^ 1));
             PW(2, mbar_wait(&bars[BI.vt_full + vb], (c / NVT) & 1));
             tc_fence_after_sync();
             const uint64_t dK = smem_desc_advance(dK0, s * L::stage_bytes), dV = smem_desc_advance(dV0, vb * L::vt_bytes);
@@ -401,7 +403,7 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
         const uint64_t dV0 = smem_desc(sm_a + L::v_off, 2 * sbo_v, sbo_v, W == 16 ? kSwz32 : kSwz64);
         for (uint32_t c = 0; c < n_chunks; ++c) {
             const uint32_t pb = c % NB, ob = c & 1, vi = c % NV;
-            PW(0, mbar_wait(&bars[BI.o2_empty + ob], ((c >> 1) & 1) ^ 1));
+            if (CS > 1 || c >= 2) PW(0, mbar_wait(&bars[BI.o2_empty + ob], ((c >> 1) & 1) ^ 1));
             PW(1, mbar_wait(&bars[BI.v_full + vi], (c / NV) & 1));
             PW(2, mbar_wait(&bars[BI.a_full + pb], (c / NB) & 1));
             tc_fence_after_sync();
@@ -659,7 +661,7 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
                         S[lg][jb][e] = fmaf(gam, S[lg][jb][e], __uint_as_float(uh[lg][4 * jb + e]) + __uint_as_float(ul[lg][4 * jb + e]));
             if (c + 1 < n_chunks) {   // version c+1 of the S operand, into the stage chunk c+1 lands in
                 const uint32_t s1 = (c + 1) % NS;
-                PW(2, mbar_wait(&bars[BI.empty + s1], ((((c + 1) / NS) & 1) ^ 1)));   // chunk c+1-NS is done with that stage
+                if (CS > 1 || c + 1 >= (uint32_t)NS) PW(2, mbar_wait(&bars[BI.empty + s1], ((((c + 1) / NS) & 1) ^ 1)));   // chunk c+1-NS is done with that stage
                 write_s_operand(s1);
                 fence_proxy_async_smem();
                 __syncwarp();
