@@ -15,6 +15,8 @@
 // moved with 16-byte vector loads/stores (L1 no-allocate), all loads of a thread issued before
 // its first store; 8 resident CTAs x 256 threads x 2 x 16 B = 64 KiB in flight per SM.
 // Odd tails and unaligned pointers take a byte path.
+#include <string.h>
+
 #include "esc_internal.h"
 
 namespace esc {
@@ -92,30 +94,50 @@ __device__ __forceinline__ void copy_tile(const uint8_t* __restrict__ src, uint8
     }
 }
 
+// Programmatic dependent launch (both directions): a copy kernel may be placed while its predecessor on the stream drains
+// (nothing is read or written before griddepcontrol.wait), and it lets its successor be placed while its own last wave drains
+// (launch_dependents once this CTA's loads are in flight; the successor's own wait still orders it after ALL of this grid's
+// stores).  Back-to-back verbs and the restore -> first suffix scan hand-over lose the launch gap (r02).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <bool kWaitFirst>
 __device__ __forceinline__ void copy_body(const CopyTable& t) {
+    // kWaitFirst: the table itself is in global memory (graph restore node) and may only be read after the dependency wait;
+    // a table in kernel-parameter space is searched BEFORE the wait, so that the loads go out the moment the wait returns
+    if (kWaitFirst) pdl_wait();
     const uint32_t n_tiles = t.n_tiles, n_seg = t.n_seg;
+    bool waited = kWaitFirst;
     for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const uint32_t e = find_entry(t.tile_begin, n_seg, tile);
         const uint64_t off = (uint64_t)(tile - t.tile_begin[e]) * kCopyTileBytes;
         const uint64_t left = t.bytes[e] - off;
         uint8_t* d = t.dst[e] + off;
-        copy_tile<1>(t.src[e] + off, &d, 1, left < kCopyTileBytes ? left : kCopyTileBytes);
+        const uint8_t* sp = t.src[e] + off;
+        if (!waited) {
+            pdl_wait();
+            waited = true;
+        }
+        copy_tile<1>(sp, &d, 1, left < kCopyTileBytes ? left : kCopyTileBytes);
     }
+    if (!waited) pdl_wait();
+    pdl_launch_dependents();
 }
 
 // table in kernel-parameter space: no H2D copy, no device allocation per verb
 __global__ void __launch_bounds__(kCopyThreads, kCopyBlocksPerSM) esc_copy_kernel(const __grid_constant__ CopyTable t) {
-    copy_body(t);
+    copy_body<false>(t);
 }
 
 // table in global memory: the restore node of a captured graph (PAPER.md:110,128 — the host
 // overwrites the bound table between replays; the graph is never recaptured)
 __global__ void __launch_bounds__(kCopyThreads, kCopyBlocksPerSM) esc_copy_indirect_kernel(const CopyTable* __restrict__ tp) {
-    copy_body(*tp);
+    copy_body<true>(*tp);
 }
 
 // fork: read each tile once, write it to n_dst live sets
 __global__ void __launch_bounds__(kCopyThreads, kCopyBlocksPerSM) esc_fork_kernel(const __grid_constant__ ForkTable t) {
+    pdl_wait();
     const uint32_t n_tiles = t.n_tiles, n_seg = t.n_seg, n_dst = t.n_dst;
     for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const uint32_t e = find_entry(t.tile_begin, n_seg, tile);
@@ -126,11 +148,27 @@ __global__ void __launch_bounds__(kCopyThreads, kCopyBlocksPerSM) esc_fork_kerne
         for (int i = 0; i < (int)ESC_MAX_FORK; ++i) d[i] = i < (int)n_dst ? t.dst[i][e] + off : nullptr;
         copy_tile<ESC_MAX_FORK>(t.src[e] + off, d, n_dst, left < kCopyTileBytes ? left : kCopyTileBytes);
     }
+    pdl_launch_dependents();
 }
 
 // ---- host -----------------------------------------------------------------------------------
 // one CTA per tile; the kernels' grid-stride loop only matters beyond the grid-size limit
 uint32_t copy_grid_blocks(uint64_t n_tiles) { return n_tiles < 0x7FFFFFFFull ? (n_tiles ? (uint32_t)n_tiles : 1u) : 0x7FFFFFFFu; }
+
+template <typename K, typename... Args>
+static cudaError_t launch_pdl(K kernel, uint32_t grid, cudaStream_t stream, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kCopyThreads);
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    memset(attr, 0, sizeof attr);
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
 
 static uint32_t fill_tiles(uint32_t* tile_begin, const uint64_t* bytes, uint32_t n) {
     uint64_t t = 0;
@@ -161,8 +199,7 @@ int launch_copy(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* d
         build_copy_table(&t, src + first, dst + first, bytes + first, m);
         if (t.n_tiles == 0) continue;
         (void)ctx;
-        esc_copy_kernel<<<copy_grid_blocks(t.n_tiles), kCopyThreads, 0, stream>>>(t);
-        ESC_CUDA(cudaGetLastError());
+        ESC_CUDA(launch_pdl(esc_copy_kernel, copy_grid_blocks(t.n_tiles), stream, t));
     }
     return ESC_OK;
 }
@@ -186,8 +223,7 @@ int launch_table_store(const CopyTable& t, CopyTable* table_dev, cudaStream_t st
 
 int launch_copy_indirect(const esc_ctx* ctx, const CopyTable* table_dev, uint32_t grid_blocks, cudaStream_t stream) {
     (void)ctx;
-    esc_copy_indirect_kernel<<<grid_blocks, kCopyThreads, 0, stream>>>(table_dev);
-    ESC_CUDA(cudaGetLastError());
+    ESC_CUDA(launch_pdl(esc_copy_indirect_kernel, grid_blocks, stream, table_dev));
     return ESC_OK;
 }
 
@@ -207,8 +243,7 @@ int launch_fork(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* c
         }
         if (t.n_tiles == 0) continue;
         (void)ctx;
-        esc_fork_kernel<<<copy_grid_blocks(t.n_tiles), kCopyThreads, 0, stream>>>(t);
-        ESC_CUDA(cudaGetLastError());
+        ESC_CUDA(launch_pdl(esc_fork_kernel, copy_grid_blocks(t.n_tiles), stream, t));
     }
     return ESC_OK;
 }

@@ -65,6 +65,7 @@ __device__ __forceinline__ void put_codes8(uint8_t* d8, uint8_t* d16, uint32_t i
 __device__ __forceinline__ uint16_t expand1(uint8_t code, float scale) { return (uint16_t)(expand2(code, scale) & 0xFFFFu); }
 
 __global__ void __launch_bounds__(kCopyThreads, 8) esc_stage_kernel(const __grid_constant__ StageTable t) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");   // programmatic dependent launch, as in copy_kernel.cu
     const uint32_t tid = threadIdx.x;
     for (uint32_t tile = blockIdx.x; tile < t.n_tiles; tile += gridDim.x) {
         uint32_t lo = 0, hi = t.n_seg;   // largest e with tile_begin[e] <= tile
@@ -101,6 +102,7 @@ __global__ void __launch_bounds__(kCopyThreads, 8) esc_stage_kernel(const __grid
             if (d16) reinterpret_cast<uint16_t*>(d16)[i] = expand1(c, scale);
         }
     }
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
 int launch_stage(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* dst8, uint8_t* const* dst16,
@@ -124,8 +126,17 @@ int launch_stage(const esc_ctx* ctx, const uint8_t* const* src, uint8_t* const* 
         t.tile_begin[m] = (uint32_t)tiles;
         t.n_tiles = (uint32_t)tiles;
         if (tiles == 0) continue;
-        esc_stage_kernel<<<copy_grid_blocks(tiles), kCopyThreads, 0, stream>>>(t);
-        ESC_CUDA(cudaGetLastError());
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(copy_grid_blocks(tiles));
+        cfg.blockDim = dim3(kCopyThreads);
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        memset(attr, 0, sizeof attr);
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        ESC_CUDA(cudaLaunchKernelEx(&cfg, esc_stage_kernel, t));
     }
     return ESC_OK;
 }
