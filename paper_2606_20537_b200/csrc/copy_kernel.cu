@@ -212,12 +212,13 @@ __global__ void __launch_bounds__(kCopyThreads) esc_table_store_kernel(const __g
     static_assert(sizeof(CopyTable) % 4 == 0, "word copy");
     const uint32_t* s = reinterpret_cast<const uint32_t*>(&t);
     uint32_t* d = reinterpret_cast<uint32_t*>(dst);
+    pdl_wait();   // a replay that still reads the previous table has completed
     for (uint32_t i = threadIdx.x; i < sizeof(CopyTable) / 4; i += kCopyThreads) d[i] = s[i];
+    pdl_launch_dependents();
 }
 
 int launch_table_store(const CopyTable& t, CopyTable* table_dev, cudaStream_t stream) {
-    esc_table_store_kernel<<<1, kCopyThreads, 0, stream>>>(t, table_dev);
-    ESC_CUDA(cudaGetLastError());
+    ESC_CUDA(launch_pdl(esc_table_store_kernel, 1, stream, t, table_dev));
     return ESC_OK;
 }
 
