@@ -10,13 +10,13 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
-SOURCES = ["esc_host.cu", "copy_kernel.cu", "stage.cu", "scan_api.cu", "scan_kernel.cu", "gdn_kernel.cu", "gdn_mma_kernel.cu", "graph.cu"]
+SOURCES = ["esc_host.cu", "copy_kernel.cu", "stage.cu", "scan_api.cu", "scan_kernel.cu", "gdn_kernel.cu", "gdn_scan_kernel.cu", "graph.cu"]
 HEADERS = [os.path.join(ROOT, "include", "esc.h"), os.path.join(CSRC, "esc_internal.h"), os.path.join(CSRC, "sm100_ptx.cuh")]
 TARGET = os.path.join(PKG, "libesc.so")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-DESC_BUILD",] + (["-DESC_TC_TRACE"] if os.environ.get("ESC_TC_TRACE") else []) + (["-DESC_SCAN_PROF"] if os.environ.get("ESC_SCAN_PROF") else []) + [
+    "-Xcompiler", "-fPIC", "-DESC_BUILD",] + (["-DESC_TC_TRACE"] if os.environ.get("ESC_TC_TRACE") else []) + (["-DESC_SCAN_PROF"] if os.environ.get("ESC_SCAN_PROF") else []) + (["-DESC_GDN_PROF"] if os.environ.get("ESC_GDN_PROF") else []) + [
     "-I", os.path.join(ROOT, "include"), "-I", CSRC,
 ]
 

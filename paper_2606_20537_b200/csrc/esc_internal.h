@@ -189,7 +189,7 @@ bool decode_key(esc_shape_key key, ScanShape* s);
 uint32_t scan_tile_columns(const esc_ctx* ctx, const ScanShape& s);
 int launch_scan(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g,
                 const float* state_in, float* state_out, void* o, uint64_t T, uint64_t t_stride, cudaStream_t stream);
-// gated delta rule, chunked form on warp-level MMAs (gdn_mma_kernel.cu)
+// gated delta rule, chunked (WY) form on tcgen05 (gdn_scan_kernel.cu)
 int launch_gdn_mma(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* beta,
                    const float* state_in, float* state_out, float* o, uint64_t T, uint64_t t_stride, cudaStream_t stream);
 

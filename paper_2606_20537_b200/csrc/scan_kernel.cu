@@ -50,6 +50,7 @@
 
 #include "esc_internal.h"
 #include "sm100_ptx.cuh"
+#include "tmap.h"
 
 namespace esc {
 
@@ -157,22 +158,6 @@ __device__ __forceinline__ constexpr ScanBars scan_bars() {
     return b;
 }
 
-__device__ __forceinline__ uint32_t pack_bf16(float lo_elem, float hi_elem) {   // element 0 in the low half
-    __nv_bfloat162 p = __floats2bfloat162_rn(lo_elem, hi_elem);
-    return *reinterpret_cast<uint32_t*>(&p);
-}
-// two-term split of a pair: returns packed hi terms, writes packed lo terms
-__device__ __forceinline__ uint32_t split2(float x0, float x1, uint32_t& lo) {
-    const uint32_t hi = pack_bf16(x0, x1);   // one cvt.rn.bf16x2.f32
-    lo = pack_bf16(x0 - __uint_as_float(hi << 16), x1 - __uint_as_float(hi & 0xFFFF0000u));
-    return hi;
-}
-__device__ __forceinline__ float ex2(float x) {
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
 template <typename OutT>
 __device__ __forceinline__ void store_o2(OutT* p, float x0, float x1);
 template <>
@@ -203,7 +188,9 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sm + L::bar_off + 64 * 8);
     float* gate = reinterpret_cast<float*>(sm + L::gate_off);   // [2][2][256]: b2 then eb per slot
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // (the shuffle tells the compiler that the warp index is warp-uniform: the role branches become uniform branches, and inside
+    // them descriptors, barrier addresses and loop state live in uniform registers instead of being moved there before every MMA)
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     uint32_t rank = 0;
     if constexpr (CS > 1) rank = cluster_ctarank();   // clusters are CS consecutive d_v slices (blockIdx.x) of one (b, h)
     const uint32_t bh = blockIdx.y, b = bh / H, h = bh % H, dv0 = blockIdx.x * W;
@@ -252,7 +239,7 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
     if constexpr (CS > 1) cluster_sync();
     else __syncthreads();
     tc_fence_after_sync();
-    const uint32_t tb = *tmem_slot;
+    const uint32_t tb = __shfl_sync(0xffffffffu, *tmem_slot, 0);
     asm volatile("griddepcontrol.wait;" ::: "memory");   // ---- global memory may be touched from here on ----
     PROF_DECL
 
@@ -707,7 +694,7 @@ static TmapEncodeFn tmap_encode_fn() {
 
 // 4-D map over a [B, t_stride, H, D] bf16 tensor whose first `T` tokens per batch row are valid:
 // dims (D, H, T, B), box (box_d, 1, box_t, 1).  Rows beyond T read as zero (the short last chunk).
-static int make_tmap(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, uint64_t T, uint64_t t_stride, uint32_t B,
+int make_tmap(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, uint64_t T, uint64_t t_stride, uint32_t B,
                      uint32_t box_d, uint32_t box_t, CUtensorMapSwizzle sw) {
     TmapEncodeFn enc = tmap_encode_fn();
     if (!enc) return ESC_ERR_CUDA;
@@ -722,7 +709,7 @@ static int make_tmap(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, u
 }
 
 // whole Q tiles for the cluster-free launch: dimensions (d % 64, t, d / 64, h, b), box (64, box_t, D / 64, 1, 1)
-static int make_tmap_halves(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, uint64_t T, uint64_t t_stride, uint32_t B,
+int make_tmap_halves(CUtensorMap* m, const void* base, uint32_t D, uint32_t H, uint64_t T, uint64_t t_stride, uint32_t B,
                             uint32_t box_t) {
     TmapEncodeFn enc = tmap_encode_fn();
     if (!enc) return ESC_ERR_CUDA;

@@ -1,7 +1,7 @@
 """-m gpu parity of esc_gdn_scan (gated delta rule) and esc_causal_conv (convolution state) through the C ABI against
 oracle/gdn_oracle.c (reading 25).  Same bars as the linear-attention scan: o within 2e-3
 (inf-norm ratio), S within 1e-3 (relative Frobenius); restore + continue bit-identical to the cold run at every boundary
-that is a multiple of the kernel's 16-token chunk (every chunk-aligned boundary), within the gates elsewhere."""
+that is a multiple of the kernel's (= the key's) 64-token chunk, within the gates elsewhere."""
 import numpy as np
 import pytest
 import torch
@@ -39,7 +39,7 @@ def run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv, s0=None, t0=0, n=None):
 
 @pytest.mark.parametrize("B,H,dk,dv,T,gate", [
     (1, 2, 64, 64, 256, "fast"),
-    (2, 3, 128, 128, 300, "fast"),       # ragged: 300 = 4 staged blocks + 44
+    (2, 3, 128, 128, 300, "fast"),       # ragged: 300 = 4 chunks + 44
     (1, 16, 128, 128, 512, "slow"),      # config-1 head shape, slow decay: the carried state matters throughout
     (1, 2, 128, 64, 1, "fast"),
     (1, 1, 64, 128, 65, "one"),
@@ -63,11 +63,11 @@ def test_gdn_restore_continue_bit_identical_at_chunk_boundaries(esc, ctx):
     beta = to_dev(synth.gdn_beta(B, T, H, seed_ids=(72,)))
     dev_in = scan_dev_inputs(si)
     o_cold, s_cold, _ = run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv)
-    for P in (64, 128, 192, 320, 16, 304):   # chunk-aligned (64) boundaries, on and off the staging-block grid; 16-token multiples
+    for P in (64, 128, 192, 256, 320):       # chunk-aligned (64) boundaries, on and off the 256-token gate-batch grid
         _, s_p, _ = run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv, n=P)
         o_b, s_t, _ = run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv, s0=s_p, t0=P)
         assert bits_equal(o_b, o_cold[:, P:]) and bits_equal(s_t, s_cold), P
-    for P in (101, 332):                     # misaligned: a different chunk grid, the same function to rounding
+    for P in (16, 304, 101, 332):            # misaligned: a different chunk grid, the same function to rounding
         _, s_p, _ = run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv, n=P)
         o_b, s_t, _ = run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv, s0=s_p, t0=P)
         assert err_o(o_b.cpu().numpy(), o_cold[:, P:].cpu().numpy().astype(np.float64)) <= 1e-4, P
