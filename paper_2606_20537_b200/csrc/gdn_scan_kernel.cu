@@ -627,14 +627,14 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             uint8_t* rop = sm + L::r_off;
 #pragma unroll
             for (int jb = 0; jb < 2; ++jb) {
-                const float xa0 = __uint_as_float(xh[4 * jb + 0]) + __uint_as_float(xl[4 * jb + 0]);
-                const float xa1 = __uint_as_float(xh[4 * jb + 1]) + __uint_as_float(xl[4 * jb + 1]);
-                const float xb0 = __uint_as_float(xh[4 * jb + 2]) + __uint_as_float(xl[4 * jb + 2]);
-                const float xb1 = __uint_as_float(xh[4 * jb + 3]) + __uint_as_float(xl[4 * jb + 3]);
-                const float r0 = bea * fmaf(-ga, xa0, __uint_as_float(va[jb] << 16));
-                const float r1 = bea * fmaf(-ga, xa1, __uint_as_float(va[jb] & 0xFFFF0000u));
-                const float r2 = beb * fmaf(-gb, xb0, __uint_as_float(vb[jb] << 16));
-                const float r3 = beb * fmaf(-gb, xb1, __uint_as_float(vb[jb] & 0xFFFF0000u));
+                // (packed fp32: FADD2 / FFMA2 / FMUL2 on the pairs of columns)
+                const float2 xa = fadd2(make_float2(__uint_as_float(xh[4 * jb + 0]), __uint_as_float(xh[4 * jb + 1])),
+                                        make_float2(__uint_as_float(xl[4 * jb + 0]), __uint_as_float(xl[4 * jb + 1])));
+                const float2 xb = fadd2(make_float2(__uint_as_float(xh[4 * jb + 2]), __uint_as_float(xh[4 * jb + 3])),
+                                        make_float2(__uint_as_float(xl[4 * jb + 2]), __uint_as_float(xl[4 * jb + 3])));
+                const float2 ra2 = fmul2(make_float2(bea, bea), ffma2(make_float2(-ga, -ga), xa, make_float2(__uint_as_float(va[jb] << 16), __uint_as_float(va[jb] & 0xFFFF0000u))));
+                const float2 rb2 = fmul2(make_float2(beb, beb), ffma2(make_float2(-gb, -gb), xb, make_float2(__uint_as_float(vb[jb] << 16), __uint_as_float(vb[jb] & 0xFFFF0000u))));
+                const float r0 = ra2.x, r1 = ra2.y, r2 = rb2.x, r3 = rb2.y;
                 uint32_t lo0, lo1;
                 const uint32_t hi0 = split2(r0, r1, lo0), hi1 = split2(r2, r3, lo1);
                 *reinterpret_cast<uint32_t*>(rop + jb * L::op_sbo + op_a) = hi0;
@@ -661,12 +661,14 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             uint8_t* wt = sm + L::wt_off;
 #pragma unroll
             for (int jb = 0; jb < 2; ++jb) {
-                const float w0 = __uint_as_float(wa[4 * jb + 0]) + __uint_as_float(wb[4 * jb + 0]);
-                const float w1 = __uint_as_float(wa[4 * jb + 1]) + __uint_as_float(wb[4 * jb + 1]);
-                const float w2 = __uint_as_float(wa[4 * jb + 2]) + __uint_as_float(wb[4 * jb + 2]);
-                const float w3 = __uint_as_float(wa[4 * jb + 3]) + __uint_as_float(wb[4 * jb + 3]);
+                const float2 wA = fadd2(make_float2(__uint_as_float(wa[4 * jb + 0]), __uint_as_float(wa[4 * jb + 1])),
+                                        make_float2(__uint_as_float(wb[4 * jb + 0]), __uint_as_float(wb[4 * jb + 1])));
+                const float2 wB = fadd2(make_float2(__uint_as_float(wa[4 * jb + 2]), __uint_as_float(wa[4 * jb + 3])),
+                                        make_float2(__uint_as_float(wb[4 * jb + 2]), __uint_as_float(wb[4 * jb + 3])));
+                const float w0 = wA.x, w1 = wA.y, w2 = wB.x, w3 = wB.y;
+                const float2 sA = fmul2(make_float2(la, la), wA), sB = fmul2(make_float2(lb, lb), wB);
                 uint32_t lo0, lo1;
-                uint32_t hi0 = split2(la * w0, la * w1, lo0), hi1 = split2(lb * w2, lb * w3, lo1);
+                uint32_t hi0 = split2(sA.x, sA.y, lo0), hi1 = split2(sB.x, sB.y, lo1);
                 *reinterpret_cast<uint32_t*>(wt + jb * L::op_sbo + op_a) = hi0;
                 *reinterpret_cast<uint32_t*>(wt + (jb + 2) * L::op_sbo + op_a) = lo0;
                 *reinterpret_cast<uint32_t*>(wt + jb * L::op_sbo + op_b) = hi1;
@@ -852,8 +854,13 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
 #pragma unroll
                 for (int jb = 0; jb < 2; ++jb)
 #pragma unroll
-                    for (int e = 0; e < 4; ++e)
-                        S[lg][jb][e] = fmaf(gam, S[lg][jb][e], __uint_as_float(uh[lg][4 * jb + e]) + __uint_as_float(ul[lg][4 * jb + e]));
+                    for (int e = 0; e < 4; e += 2) {
+                        const float2 u = fadd2(make_float2(__uint_as_float(uh[lg][4 * jb + e]), __uint_as_float(uh[lg][4 * jb + e + 1])),
+                                               make_float2(__uint_as_float(ul[lg][4 * jb + e]), __uint_as_float(ul[lg][4 * jb + e + 1])));
+                        const float2 sn = ffma2(make_float2(gam, gam), make_float2(S[lg][jb][e], S[lg][jb][e + 1]), u);
+                        S[lg][jb][e] = sn.x;
+                        S[lg][jb][e + 1] = sn.y;
+                    }
             if (c + 1 < n_chunks) {
                 // operand buffer (c + 1) % 2 was last read by X(c - 1), Y(c - 1): complete, they were issued before U(c) by the same thread
                 write_s_operand((c + 1) & 1);

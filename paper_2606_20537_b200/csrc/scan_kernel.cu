@@ -433,8 +433,8 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
                 uint32_t hi[4], lo[4];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const float x0 = __uint_as_float(w[e] << 16) * sc, x1 = __uint_as_float(w[e] & 0xFFFF0000u) * sc;
-                    hi[e] = split2(x0, x1, lo[e]);
+                    const float2 x = fmul2(make_float2(__uint_as_float(w[e] << 16), __uint_as_float(w[e] & 0xFFFF0000u)), make_float2(sc, sc));
+                    hi[e] = split2(x.x, x.y, lo[e]);
                 }
                 const uint32_t off = cg * L::sbo_vt + (j >> 3) * 128 + (j & 7) * 16;
                 *reinterpret_cast<uint4*>(vt + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
@@ -481,10 +481,12 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
                 if (ks <= q) {
 #pragma unroll
                     for (int j = 0; j < 2; ++j) {
-                        float a0 = __uint_as_float(r[e][4 * j + 0]) * ex2(bia - bj[e][j].x);
-                        float a1 = __uint_as_float(r[e][4 * j + 1]) * ex2(bia - bj[e][j].y);
-                        float c0 = __uint_as_float(r[e][4 * j + 2]) * ex2(bib - bj[e][j].x);
-                        float c1 = __uint_as_float(r[e][4 * j + 3]) * ex2(bib - bj[e][j].y);
+                        // (packed fp32: one FADD2 / FMUL2 per pair of columns)
+                        const float2 nbj = make_float2(-bj[e][j].x, -bj[e][j].y);
+                        const float2 xa = fadd2(make_float2(bia, bia), nbj), xc = fadd2(make_float2(bib, bib), nbj);
+                        const float2 pa = fmul2(make_float2(__uint_as_float(r[e][4 * j + 0]), __uint_as_float(r[e][4 * j + 1])), make_float2(ex2(xa.x), ex2(xa.y)));
+                        const float2 pc = fmul2(make_float2(__uint_as_float(r[e][4 * j + 2]), __uint_as_float(r[e][4 * j + 3])), make_float2(ex2(xc.x), ex2(xc.y)));
+                        float a0 = pa.x, a1 = pa.y, c0 = pc.x, c1 = pc.y;
                         if (ks == q) {   // the diagonal step: causal mask j <= i
                             const int j0 = 16 * ks + 8 * j + 2 * (lane & 3);
                             a0 = (j0 <= ra) ? a0 : 0.f;
@@ -534,7 +536,11 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
                 tmem_ld_16x256b_x2(tmem_addr(tb, lane_base, L::tm_po + pb * NPO + kC + W + 16 * cg), r1l);
                 tmem_ld_wait();
 #pragma unroll
-                for (int i = 0; i < 8; ++i) o1[cg][i] = __uint_as_float(r1h[i]) + __uint_as_float(r1l[i]);
+                for (int i = 0; i < 8; i += 2) {
+                    const float2 t = fadd2(make_float2(__uint_as_float(r1h[i]), __uint_as_float(r1h[i + 1])), make_float2(__uint_as_float(r1l[i]), __uint_as_float(r1l[i + 1])));
+                    o1[cg][i] = t.x;
+                    o1[cg][i + 1] = t.y;
+                }
             }
             tc_fence_before_sync();
             __syncwarp();
@@ -559,10 +565,12 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
             for (int cg = 0; cg < W / 16; ++cg)
 #pragma unroll
                 for (int jb = 0; jb < 2; ++jb) {   // columns 16 cg + 8 jb + 2 (t % 4) + {0, 1}
-                    if (ra < n) store_o2<OutT>(oa + 16 * cg + jb * 8, fmaf(ea, o1[cg][4 * jb + 0], __uint_as_float(r2[cg][4 * jb + 0])),
-                                               fmaf(ea, o1[cg][4 * jb + 1], __uint_as_float(r2[cg][4 * jb + 1])));
-                    if (rb < n) store_o2<OutT>(oc + 16 * cg + jb * 8, fmaf(ebb, o1[cg][4 * jb + 2], __uint_as_float(r2[cg][4 * jb + 2])),
-                                               fmaf(ebb, o1[cg][4 * jb + 3], __uint_as_float(r2[cg][4 * jb + 3])));
+                    const float2 va = ffma2(make_float2(ea, ea), make_float2(o1[cg][4 * jb + 0], o1[cg][4 * jb + 1]),
+                                            make_float2(__uint_as_float(r2[cg][4 * jb + 0]), __uint_as_float(r2[cg][4 * jb + 1])));
+                    const float2 vc = ffma2(make_float2(ebb, ebb), make_float2(o1[cg][4 * jb + 2], o1[cg][4 * jb + 3]),
+                                            make_float2(__uint_as_float(r2[cg][4 * jb + 2]), __uint_as_float(r2[cg][4 * jb + 3])));
+                    if (ra < n) store_o2<OutT>(oa + 16 * cg + jb * 8, va.x, va.y);
+                    if (rb < n) store_o2<OutT>(oc + 16 * cg + jb * 8, vc.x, vc.y);
                 }
             if (q == 3 && lane == 0) TC_TRACE(8, c);
         }
@@ -644,8 +652,13 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
 #pragma unroll
                 for (int jb = 0; jb < 2; ++jb)
 #pragma unroll
-                    for (int e = 0; e < 4; ++e)
-                        S[lg][jb][e] = fmaf(gam, S[lg][jb][e], __uint_as_float(uh[lg][4 * jb + e]) + __uint_as_float(ul[lg][4 * jb + e]));
+                    for (int e = 0; e < 4; e += 2) {
+                        const float2 u = fadd2(make_float2(__uint_as_float(uh[lg][4 * jb + e]), __uint_as_float(uh[lg][4 * jb + e + 1])),
+                                               make_float2(__uint_as_float(ul[lg][4 * jb + e]), __uint_as_float(ul[lg][4 * jb + e + 1])));
+                        const float2 sn = ffma2(make_float2(gam, gam), make_float2(S[lg][jb][e], S[lg][jb][e + 1]), u);
+                        S[lg][jb][e] = sn.x;
+                        S[lg][jb][e + 1] = sn.y;
+                    }
             if (c + 1 < n_chunks) {   // version c+1 of the S operand, into the stage chunk c+1 lands in
                 const uint32_t s1 = (c + 1) % NS;
                 if (CS > 1 || c + 1 >= (uint32_t)NS) PW(2, mbar_wait(&bars[BI.empty + s1], ((((c + 1) / NS) & 1) ^ 1)));   // chunk c+1-NS is done with that stage

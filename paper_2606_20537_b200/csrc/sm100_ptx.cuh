@@ -49,6 +49,9 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 // (a suspend-time hint or a nanosleep back-off in this loop changed nothing measurable: r01 experiments)
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) {
+#ifdef ESC_MBAR_BACKOFF
+        asm volatile("nanosleep.u32 %0;" ::"r"((uint32_t)ESC_MBAR_BACKOFF));
+#endif
     }
 }
 
@@ -363,6 +366,28 @@ __host__ __device__ constexpr uint32_t idesc_bf16(uint32_t M, uint32_t N, uint32
 
 }  // namespace ptx
 
+// ---- packed fp32 arithmetic (sm_100: FADD2 / FMUL2 / FFMA2, two lanes per instruction; a pair whose halves are the same
+// register is encoded as a scalar broadcast operand) -------------------------------------------------------------------
+__device__ __forceinline__ float2 fadd2(float2 a, float2 b) {
+    float2 d;
+    asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tadd.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return d;
+}
+__device__ __forceinline__ float2 fmul2(float2 a, float2 b) {
+    float2 d;
+    asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmul.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return d;
+}
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
+    float2 d;
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return d;
+}
+
 // ---- fp32 -> two-term bf16 operand splits, ex2 (shared by the tensor-core scan kernels) ----------
 __device__ __forceinline__ uint32_t pack_bf16(float lo_elem, float hi_elem) {   // element 0 in the low half
     __nv_bfloat162 p = __floats2bfloat162_rn(lo_elem, hi_elem);
@@ -371,7 +396,8 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo_elem, float hi_elem) {   
 // two-term split of a pair: returns packed hi terms, writes packed lo terms
 __device__ __forceinline__ uint32_t split2(float x0, float x1, uint32_t& lo) {
     const uint32_t hi = pack_bf16(x0, x1);   // one cvt.rn.bf16x2.f32
-    lo = pack_bf16(x0 - __uint_as_float(hi << 16), x1 - __uint_as_float(hi & 0xFFFF0000u));
+    const float2 r = fadd2(make_float2(x0, x1), make_float2(-__uint_as_float(hi << 16), -__uint_as_float(hi & 0xFFFF0000u)));
+    lo = pack_bf16(r.x, r.y);
     return hi;
 }
 __device__ __forceinline__ float ex2(float x) {
