@@ -758,10 +758,10 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
     conv_ms, _ = med_ms(lambda: esc.causal_conv(ctx, cx, cw, cst, cst, cy, 1, Tg, Tg, Cc, Wc, esc.CONV_SILU, stream=stream), n=7)
     conv_alg = Tg * Cc * 6
     res["gated_delta_rule"] = {"tokens": Tg, "ms": gdn_ms, "tokens_per_s": Tg / (gdn_ms * 1e-3),
-                               "roofline": {"kernel": "esc_gdn_mma_kernel<128> (chunked WY form, 16-token chunks, warp-level MMAs, B1 H16 d128)", "bound": "hbm",
+                               "roofline": {"kernel": "esc_gdn_scan_kernel<128> (chunked WY form, 64-token chunks, tcgen05 / TMEM / TMA, B1 H16 d128)", "bound": "hbm",
                                             "achieved": gdn_alg / (gdn_ms * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
                                             "frac": gdn_alg / (gdn_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "alg_bytes_per_launch": gdn_alg,
-                                            "note": "bound by the per-chunk dependency chain of the recurrence warps (one CTA per (b, h, 16 d_v columns)), not HBM"},
+                                            "note": "bound by the per-chunk dependency chain S -> X -> R -> Wm -> W~ -> U -> S (three MMA groups and three register passes) and by the off-chain inverse of the 64 x 64 triangular system, one CTA per (b, h, 16 d_v columns); not HBM"},
                                "causal_conv": {"channels": Cc, "window": Wc, "us": conv_ms * 1e3, "GBps": conv_alg / (conv_ms * 1e-3) / 1e9,
                                                "frac_of_measured_peak": conv_alg / (conv_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
                                                "alg_bytes": "2 B read + 4 B written per element"}}

@@ -5,8 +5,15 @@
 #include <cuda_bf16.h>
 
 #include "esc_internal.h"
+#include "sm100_ptx.cuh"
 
 namespace esc {
+
+__device__ __forceinline__ float rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 
 // ---- short causal depthwise convolution, window W <= 8 -----------------------------------------------------
 // Bound: HBM (2 B read + 4 B written per element).  A thread owns 4 consecutive channels (one 8-byte bf16 vector; a
@@ -78,13 +85,20 @@ __global__ void __launch_bounds__(kConvThreads) esc_causal_conv_kernel(const __n
         for (int u = 0; u < U; ++u) {
             if (t + u < n_tok) {
                 bf16x4_to_f32(raw[u], win[W - 1]);
+                // two channels per instruction (sm_100 packed fp32: FFMA2 / FMUL2 / FADD2); same roundings as the scalar forms
                 float acc[P];
 #pragma unroll
-                for (int j = 0; j < P; ++j) {
-                    float s_ = 0.f;
+                for (int j = 0; j < P; j += 2) {
+                    float2 s2 = make_float2(0.f, 0.f);
 #pragma unroll
-                    for (int i = 0; i < W; ++i) s_ = fmaf(wt[i][j], win[i][j], s_);
-                    acc[j] = silu ? __fdividef(s_, 1.f + __expf(-s_)) : s_;
+                    for (int i = 0; i < W; ++i) s2 = ffma2(make_float2(wt[i][j], wt[i][j + 1]), make_float2(win[i][j], win[i][j + 1]), s2);
+                    if (silu) {   // s / (1 + e^-s), e^-s = 2^(-s log2 e)
+                        const float2 t = fmul2(s2, make_float2(-1.4426950408889634f, -1.4426950408889634f));
+                        const float2 d = fadd2(make_float2(ex2(t.x), ex2(t.y)), make_float2(1.f, 1.f));
+                        s2 = fmul2(s2, make_float2(rcp_approx(d.x), rcp_approx(d.y)));
+                    }
+                    acc[j] = s2.x;
+                    acc[j + 1] = s2.y;
                 }
                 *reinterpret_cast<float4*>(yp + (size_t)u * C) = make_float4(acc[0], acc[1], acc[2], acc[3]);
 #pragma unroll

@@ -201,6 +201,7 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
     // its on-chip setup while this one runs; everything this kernel reads from or writes to global memory comes after
     // griddepcontrol.wait below, i.e. after the preceding kernel has completed and flushed.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (threadIdx.x == 0) TC_TRACE(11, 0);
 
     // commit that every CTA of the cluster must see (stage reuse: every CTA writes into every CTA's stage)
     auto commit_all = [&](uint64_t* bar) {   // warp-uniform (every lane calls it, one elected lane issues)
@@ -240,7 +241,9 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
     else __syncthreads();
     tc_fence_after_sync();
     const uint32_t tb = __shfl_sync(0xffffffffu, *tmem_slot, 0);
+    if (threadIdx.x == 0) TC_TRACE(14, 0);
     asm volatile("griddepcontrol.wait;" ::: "memory");   // ---- global memory may be touched from here on ----
+    if (threadIdx.x == 0) TC_TRACE(12, 0);
     PROF_DECL
 
     if (warp == 0) {
@@ -680,12 +683,14 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
     }
 
     PROF_END;
+    if (threadIdx.x == 0) TC_TRACE(13, 0);
     // ---- teardown: every tcgen05 op of this CTA has completed (the state and epilogue warps waited on the last commits),
     // and no peer still multicasts or arrives into this CTA once the whole cluster is here ----
     tc_fence_before_sync();
     if constexpr (CS > 1) cluster_sync_relaxed();
     else __syncthreads();
     if (warp == 2) tmem_dealloc(tb, L::tmem_cols);
+    if (threadIdx.x == 0) TC_TRACE(15, 0);
 }
 
 // ---- host ---------------------------------------------------------------------------------------
