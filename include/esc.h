@@ -287,10 +287,10 @@ int esc_linattn_scan(esc_ctx* ctx, esc_shape_key key,
  * esc_gdn_scan: for every (b,h), S_0 = state_in[b,h]:
  *      u_t = k_t (a_t S_{t-1}) ,  S_t = a_t S_{t-1} + beta_t k_t^T (v_t - u_t) ,  o_t = q_t S_t ,  state_out = S_T
  * Layouts, alignment and aliasing rules as esc_linattn_scan; `g` holds a_t in (0,1], `beta` [B, T_stride, H] fp32 in [0,1];
- * keys are expected L2-normalised by the caller.  Evaluated in the chunked (WY) form, 16 tokens at a time, on the tensor
+ * keys are expected L2-normalised by the caller.  Evaluated in the chunked (WY) form, 64 tokens at a time, on tcgen05 tensor
  * cores (fp32 state, two-term bf16 operand splits): restore + continue is bit-identical to the cold run at every boundary
- * that is a multiple of 16 tokens from the start of the sequence of calls — in particular every boundary aligned to the
- * key's chunk — and agrees to rounding elsewhere.  out_dtype must be F32.
+ * that is a multiple of 64 tokens from the start of the sequence of calls - in particular every boundary aligned to the
+ * key's chunk - and agrees to rounding elsewhere.  out_dtype must be F32.
  *
  * esc_causal_conv: depthwise causal FIR of window W (1..8) over x [B, T_stride, C] bf16 (C % 8 == 0), weights w [C, W] fp32:
  *      y_t[c] = sum_{i<W} w[c][i] * x_{t-W+1+i}[c]      (+ SiLU with ESC_CONV_SILU),   y [B, T, C] fp32 (dense in T)
