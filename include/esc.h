@@ -237,6 +237,23 @@ int esc_dequant_stage_fill(esc_bufset* live, uint32_t row, uint64_t upto_tokens,
 int esc_restore_ex(esc_bufset* live, const esc_bufset* capsule, const uint64_t* expect_prefix_digest, uint32_t flags,
                    void* stream);
 
+/* ---- restore without caller scratch and without device allocation ---------------------------------------------------
+ * esc_restore_static: esc_restore (same pairing rules, same bytes written, same position / stage bookkeeping) for callers
+ * that cannot call cudaMalloc or hand over scratch: code under someone else's stream capture, tight serving loops, harnesses
+ * that forbid allocation.  It runs the table-in-global-memory copy kernel of the graph path (esc_graph_scratch_bytes) with
+ * its descriptor tables in a static device array inside the library: 13 KiB that every GPU which loads the library holds
+ * until exit.  No cudaMalloc / cudaFree / allocating routine is called; per 112 segments one table-store launch and one copy
+ * launch on `stream`.
+ *   Limit: the (live set, boundary) pair may have at most ESC_RESTORE_STATIC_MAX_SEGMENTS (row, segment) entries, else
+ *          ESC_ERR_CAPACITY and nothing is enqueued (esc_restore has no such limit).
+ *   Sharing: every call on a device uses the same tables, which keep the last call's contents (a call rewrites every word
+ *          it uses; nothing needs clearing).  Calls are ordered by their stream; calls whose kernels may overlap on the GPU
+ *          (different streams with no event between them, different host threads) race on the tables and must be
+ *          serialised by the caller. */
+#define ESC_RESTORE_STATIC_MAX_SEGMENTS 448u
+uint32_t esc_restore_static_max_segments(void);
+int esc_restore_static(esc_bufset* live, const esc_bufset* capsule, const uint64_t* expect_prefix_digest, void* stream);
+
 /* ---- chunked gated linear-attention scan ---------------------------------------------- */
 #define ESC_DTYPE_BF16 1u
 #define ESC_DTYPE_F32  2u

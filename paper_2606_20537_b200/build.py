@@ -10,7 +10,7 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
-SOURCES = ["esc_host.cu", "copy_kernel.cu", "stage.cu", "scan_api.cu", "scan_kernel.cu", "gdn_kernel.cu", "gdn_scan_kernel.cu", "graph.cu"]
+SOURCES = ["esc_host.cu", "copy_kernel.cu", "stage.cu", "scan_api.cu", "scan_kernel.cu", "gdn_kernel.cu", "gdn_scan_kernel.cu", "graph.cu", "noalloc.cu"]
 HEADERS = [os.path.join(ROOT, "include", "esc.h"), os.path.join(CSRC, "esc_internal.h"), os.path.join(CSRC, "sm100_ptx.cuh")]
 TARGET = os.path.join(PKG, "libesc.so")
 

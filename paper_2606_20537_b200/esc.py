@@ -85,6 +85,8 @@ _sig = {
     "esc_dequant_stage_fill": (C.c_int, [_P, C.c_uint32, C.c_uint64, _P]),
     "esc_restore_ex": (C.c_int, [_P, _P, C.POINTER(C.c_uint64), C.c_uint32, _P]),
     "esc_capsule_valid_end": (C.c_int, [_P, C.c_uint32, C.POINTER(C.c_uint64)]),
+    "esc_restore_static_max_segments": (C.c_uint32, []),
+    "esc_restore_static": (C.c_int, [_P, _P, C.POINTER(C.c_uint64), _P]),
     "esc_shape_key_make": (C.c_uint64, [C.c_uint32] * 7),
     "esc_scan_tile_columns": (C.c_int, [_P, C.c_uint64, C.POINTER(C.c_uint32)]),
     "esc_linattn_scan": (C.c_int, [_P, C.c_uint64] + [_P] * 7 + [C.c_uint64, C.c_uint64, C.c_uint32, _P]),
@@ -296,6 +298,12 @@ def snapshot(live, P, chunk, storage, storage_bytes=None, prefix_digest=0, flags
 def restore(live, capsule, expect_prefix_digest=None, stream=None):
     e = None if expect_prefix_digest is None else C.byref(C.c_uint64(expect_prefix_digest))
     _check(lib.esc_restore(live.h, capsule.h, e, _stream(stream)), "esc_restore")
+
+
+def restore_static(live, capsule, expect_prefix_digest=None, stream=None):
+    """esc_restore with its descriptor tables in the library's static device array: no scratch, no device allocation."""
+    e = None if expect_prefix_digest is None else C.byref(C.c_uint64(expect_prefix_digest))
+    _check(lib.esc_restore_static(live.h, capsule.h, e, _stream(stream)), "esc_restore_static")
 
 
 def restore_ex(live, capsule, expect_prefix_digest=None, flags=0, stream=None):
