@@ -761,6 +761,7 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
                                "roofline": {"kernel": "esc_gdn_scan_kernel<128> (chunked WY form, 64-token chunks, tcgen05 / TMEM / TMA, B1 H16 d128)", "bound": "hbm",
                                             "achieved": gdn_alg / (gdn_ms * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
                                             "frac": gdn_alg / (gdn_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "alg_bytes_per_launch": gdn_alg,
+                                            "traffic": measured_traffic("esc_gdn_scan_kernel")[0], "traffic_note": measured_traffic("esc_gdn_scan_kernel")[1],
                                             "note": "bound by the per-chunk dependency chain S -> X -> R -> Wm -> W~ -> U -> S (three MMA groups and three register passes) and by the off-chain inverse of the 64 x 64 triangular system, one CTA per (b, h, 16 d_v columns); not HBM"},
                                "causal_conv": {"channels": Cc, "window": Wc, "us": conv_ms * 1e3, "GBps": conv_alg / (conv_ms * 1e-3) / 1e9,
                                                "frac_of_measured_peak": conv_alg / (conv_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
