@@ -16,7 +16,7 @@ TARGET = os.path.join(PKG, "libesc.so")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-DESC_BUILD",] + (["-DESC_TC_TRACE"] if os.environ.get("ESC_TC_TRACE") else []) + (["-DESC_SCAN_PROF"] if os.environ.get("ESC_SCAN_PROF") else []) + (["-DESC_GDN_PROF"] if os.environ.get("ESC_GDN_PROF") else []) + (["-DESC_MBAR_BACKOFF=" + os.environ["ESC_MBAR_BACKOFF"]] if os.environ.get("ESC_MBAR_BACKOFF") else []) + [
+    "-Xcompiler", "-fPIC", "-DESC_BUILD",] + (["-DESC_TC_TRACE"] if os.environ.get("ESC_TC_TRACE") else []) + (["-DESC_SCAN_PROF"] if os.environ.get("ESC_SCAN_PROF") else []) + (["-DESC_GDN_PROF"] if os.environ.get("ESC_GDN_PROF") else []) + (["-D" + x for x in os.environ.get("ESC_DEFS", "").split()]) + (["-DESC_MBAR_BACKOFF=" + os.environ["ESC_MBAR_BACKOFF"]] if os.environ.get("ESC_MBAR_BACKOFF") else []) + [
     "-I", os.path.join(ROOT, "include"), "-I", CSRC,
 ]
 

@@ -619,11 +619,6 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             tmem_ld_16x256b_x2(tmem_addr(tb, 32 * q, L::tm_x + W), xl);
             tmem_ld_wait();
             tc_fence_before_sync();
-            __syncwarp();
-            if (lane == 0) {
-                mbar_arrive(&bars[BI.x_read]);
-                mbar_arrive(&bars[BI.v_read + vi]);
-            }
             uint8_t* rop = sm + L::r_off;
 #pragma unroll
             for (int jb = 0; jb < 2; ++jb) {
@@ -644,7 +639,11 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             }
             fence_proxy_async_smem();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&bars[BI.r_full]);
+            if (lane == 0) {
+                mbar_arrive(&bars[BI.r_full]);
+                mbar_arrive(&bars[BI.x_read]);       // (X and the V tile were read before the operand was written)
+                mbar_arrive(&bars[BI.v_read + vi]);
+            }
             // ---- Wm ----
             GW_(3, mbar_wait(&bars[BI.w_done + sb], (c >> 1) & 1));
             tc_fence_after_sync();
@@ -656,25 +655,32 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars[BI.w_read]);
             if (c >= 1) GW_(4, mbar_wait(&bars[BI.u_done + ((c - 1) & 1)], ((c - 1) >> 1) & 1));   // U(c - 1) has read the W~ operand
-            if (c >= 2) GW_(5, mbar_wait(&bars[BI.o2_done + sb], ((c - 2) >> 1) & 1));             // O2(c - 2) has read Wm operand sb
             uint8_t* wv = sm + L::wv_off + sb * L::op_bytes;
             uint8_t* wt = sm + L::wt_off;
+            // the decayed W~ operand first: it is the one on the carry chain (U waits for it); the Wm operand of the outputs after it
+            float2 wA[2], wB[2];
 #pragma unroll
             for (int jb = 0; jb < 2; ++jb) {
-                const float2 wA = fadd2(make_float2(__uint_as_float(wa[4 * jb + 0]), __uint_as_float(wa[4 * jb + 1])),
-                                        make_float2(__uint_as_float(wb[4 * jb + 0]), __uint_as_float(wb[4 * jb + 1])));
-                const float2 wB = fadd2(make_float2(__uint_as_float(wa[4 * jb + 2]), __uint_as_float(wa[4 * jb + 3])),
-                                        make_float2(__uint_as_float(wb[4 * jb + 2]), __uint_as_float(wb[4 * jb + 3])));
-                const float w0 = wA.x, w1 = wA.y, w2 = wB.x, w3 = wB.y;
-                const float2 sA = fmul2(make_float2(la, la), wA), sB = fmul2(make_float2(lb, lb), wB);
+                wA[jb] = fadd2(make_float2(__uint_as_float(wa[4 * jb + 0]), __uint_as_float(wa[4 * jb + 1])),
+                               make_float2(__uint_as_float(wb[4 * jb + 0]), __uint_as_float(wb[4 * jb + 1])));
+                wB[jb] = fadd2(make_float2(__uint_as_float(wa[4 * jb + 2]), __uint_as_float(wa[4 * jb + 3])),
+                               make_float2(__uint_as_float(wb[4 * jb + 2]), __uint_as_float(wb[4 * jb + 3])));
+                const float2 sA = fmul2(make_float2(la, la), wA[jb]), sB = fmul2(make_float2(lb, lb), wB[jb]);
                 uint32_t lo0, lo1;
-                uint32_t hi0 = split2(sA.x, sA.y, lo0), hi1 = split2(sB.x, sB.y, lo1);
+                const uint32_t hi0 = split2(sA.x, sA.y, lo0), hi1 = split2(sB.x, sB.y, lo1);
                 *reinterpret_cast<uint32_t*>(wt + jb * L::op_sbo + op_a) = hi0;
                 *reinterpret_cast<uint32_t*>(wt + (jb + 2) * L::op_sbo + op_a) = lo0;
                 *reinterpret_cast<uint32_t*>(wt + jb * L::op_sbo + op_b) = hi1;
                 *reinterpret_cast<uint32_t*>(wt + (jb + 2) * L::op_sbo + op_b) = lo1;
-                hi0 = split2(w0, w1, lo0);
-                hi1 = split2(w2, w3, lo1);
+            }
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars[BI.wt_full]);
+            if (c >= 2) GW_(5, mbar_wait(&bars[BI.o2_done + sb], ((c - 2) >> 1) & 1));             // O2(c - 2) has read Wm operand sb
+#pragma unroll
+            for (int jb = 0; jb < 2; ++jb) {
+                uint32_t lo0, lo1;
+                const uint32_t hi0 = split2(wA[jb].x, wA[jb].y, lo0), hi1 = split2(wB[jb].x, wB[jb].y, lo1);
                 *reinterpret_cast<uint32_t*>(wv + jb * L::op_sbo + op_a) = hi0;
                 *reinterpret_cast<uint32_t*>(wv + (jb + 2) * L::op_sbo + op_a) = lo0;
                 *reinterpret_cast<uint32_t*>(wv + jb * L::op_sbo + op_b) = hi1;
@@ -683,7 +689,6 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) {
-                mbar_arrive(&bars[BI.wt_full]);
                 mbar_arrive(&bars[BI.wv_full + sb]);
                 if ((c % kGCPB) == (uint32_t)kGCPB - 1 || c + 1 == n_chunks) mbar_arrive(&bars[BI.g_empty + gslot]);
             }
