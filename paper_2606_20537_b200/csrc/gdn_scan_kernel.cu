@@ -40,6 +40,7 @@
 // no split-K, every accumulator produced by one issuer in a fixed order.  A restore + continue at a boundary that is a multiple
 // of 64 tokens from the start of the sequence of calls replays the same chunks: same bits as the cold run.
 #include <cuda.h>
+#include <string.h>
 #include <cuda_bf16.h>
 
 #include "esc_internal.h"
@@ -54,6 +55,13 @@ constexpr int kGC = 64;            // tokens per chunk
 constexpr int kGW = 16;            // d_v columns per CTA
 constexpr int kGBatch = 256;       // tokens per gate batch
 constexpr int kGCPB = kGBatch / kGC;
+#ifndef ESC_GDN_NS
+#define ESC_GDN_NS 3
+#endif
+#ifndef ESC_GDN_CLUSTER
+#define ESC_GDN_CLUSTER 4
+#endif
+constexpr int kGdnCluster = ESC_GDN_CLUSTER;   // d_v slices of a head that share the chunk inverses (even)
 constexpr int kGAhead = 4;         // chunks prefetched into L2 ahead of the shared-memory ring
 
 #ifdef ESC_GDN_PROF   // bring-up only: cycles every role of CTA (0,0) spends in each of its waits / sections, and in its loop in total
@@ -75,7 +83,7 @@ __device__ long long g_gdn_prof[32 * 8];
 template <int DK>
 struct GdnCfg {
     static constexpr int NH = DK / 64;                       // 64-column halves of a Q / K tile
-    static constexpr int NS = 3;                             // Q | K stages
+    static constexpr int NS = ESC_GDN_NS;                    // Q | K stages
     static constexpr int NV = 4;                             // V tiles
     static constexpr int kWarps = 28;
     static constexpr int kThreads = kWarps * 32;
@@ -92,24 +100,28 @@ struct GdnCfg {
     static constexpr uint32_t a_pitch = 144;                 // A^k | U staging matrix: row-major bf16, padded rows (conflict-free ldmatrix)
     static constexpr uint32_t a_term_bytes = kGC * a_pitch;
     static constexpr uint32_t lt_pitch = 20;                 // fp32 diagonal blocks, transposed: LT[j][i]
-    static constexpr uint32_t lt_bytes = 2 * 4 * 16 * lt_pitch * 4;   // per T-warp set
+    static constexpr uint32_t lt_bytes = 4 * 16 * lt_pitch * 4;
+    static constexpr uint32_t tg_bytes = 4 * 2 * kGC * 4;      // the T warps' own gate values of a chunk: per warp [b2[64], beta[64]]
 
     static constexpr uint32_t stage_off = 0;
     static constexpr uint32_t s_off = stage_off + NS * stage_bytes;
     static constexpr uint32_t v_off = s_off + 2 * s_bytes;
     static constexpr uint32_t t_off = v_off + NV * v_bytes;
-    static constexpr uint32_t r_off = t_off + 2 * t_bytes;
+    static constexpr uint32_t tstage_off = t_off + 2 * t_bytes;   // the T of an owned chunk, before it is pushed to the cluster
+    static constexpr uint32_t a_off = tstage_off + t_bytes;       // staging matrix [hi][lo]; first the K tile of the owned chunk (G = K K^T)
+    static constexpr uint32_t r_off = a_off + 2 * a_term_bytes;
     static constexpr uint32_t wv_off = r_off + op_bytes;     // [2]
     static constexpr uint32_t wt_off = wv_off + 2 * op_bytes;
-    static constexpr uint32_t a_off = wt_off + op_bytes;     // [hi][lo]
-    static constexpr uint32_t lt_off = a_off + 2 * 2 * a_term_bytes;   // the staging matrix is double-buffered by chunk parity
-    static constexpr uint32_t gate_off = lt_off + lt_bytes;  // [2][b2[256], eb[256], beta[256]] fp32
+    static constexpr uint32_t lt_off = wt_off + op_bytes;
+    static constexpr uint32_t tg_off = lt_off + lt_bytes;
+    static constexpr uint32_t traw_off = tg_off + tg_bytes;  // [2][a[64], beta[64]] fp32: raw gate inputs of the owned chunks (cp.async, one ahead)
+    static constexpr uint32_t gate_off = traw_off + 2 * 2 * kGC * 4;  // [2][b2[256], eb[256], beta[256]] fp32
     static constexpr uint32_t raw_off = gate_off + 2 * 3 * kGBatch * 4;   // [2][a[256], beta[256]] fp32: the gate warp's staging
     static constexpr uint32_t bar_off = raw_off + 2 * 2 * kGBatch * 4;
     static constexpr uint32_t total = bar_off + 64 * 8 + 16 + 1024;
     // TMEM columns
     static constexpr uint32_t tm_p = 0;        // [2] x 64: P -> A^q hi | lo
-    static constexpr uint32_t tm_g = 128;      // [2] x 64: G
+    static constexpr uint32_t tm_g = 128;      // 64: G of the chunk this CTA inverts (192..255 unused)
     static constexpr uint32_t tm_x = 256;      // 32: X hi | lo
     static constexpr uint32_t tm_y = 288;      // [2] x 32: Y hi | lo
     static constexpr uint32_t tm_w = 352;      // 32: T_hi R_hi + T_lo R_hi | T_hi R_lo
@@ -117,11 +129,12 @@ struct GdnCfg {
     static constexpr uint32_t tm_u = 448;      // [2] x 32: U hi | lo
     static constexpr uint32_t tmem_cols = 512;
     static_assert(stage_bytes % 1024 == 0 && s_off % 1024 == 0 && s_half_bytes % 1024 == 0 && v_off % 1024 == 0, "swizzled regions: 1024-byte alignment");
+    static_assert(a_off % 1024 == 0 && 2 * a_term_bytes >= q_bytes, "the K tile of an owned chunk lands in the staging matrix");
     static_assert(total <= 232448, "shared memory budget");
 };
 
 struct GdnBars {
-    int full, empty, v_full, v_read, s_full, g_done, g_read, p_done, a_full, x_done, x_read, y_done, y_free, t_full, r_full, w_done,
+    int full, empty, v_full, v_read, s_full, g_done, kg_full, t_free, t_ack, p_done, a_full, x_done, x_read, y_done, y_free, t_full, r_full, w_done,
         w_read, wv_full, wt_full, o2_done, o2_free, u_done, u_empty, g_full, g_empty, row_ready, count;
 };
 template <int DK>
@@ -134,8 +147,10 @@ __device__ __forceinline__ constexpr GdnBars gdn_bars() {
     b.v_full = i; i += L::NV;
     b.v_read = i; i += L::NV;
     b.s_full = i; i += 2;
-    b.g_done = i; i += 2;
-    b.g_read = i; i += 2;
+    b.g_done = i; i += 1;
+    b.kg_full = i; i += 1;
+    b.t_free = i; i += 2;
+    b.t_ack = i; i += 1;
     b.p_done = i; i += 2;
     b.a_full = i; i += 2;
     b.x_done = i; i += 1;
@@ -154,7 +169,7 @@ __device__ __forceinline__ constexpr GdnBars gdn_bars() {
     b.u_empty = i; i += 2;
     b.g_full = i; i += 2;
     b.g_empty = i; i += 2;
-    b.row_ready = i; i += 8;
+    b.row_ready = i; i += 4;
     b.count = i;
     return b;
 }
@@ -183,6 +198,9 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
     const uint32_t n_chunks = (uint32_t)((T + kGC - 1) / kGC);
     const int q = warp & 3;   // TMEM lane quadrant this warp may access
     const int g8 = lane >> 2, t4 = lane & 3;
+    // the d_v slices of one (b, h) form a thread-block cluster: T = (I + A^k)^-1 depends on k, beta and the decays only, so CTA
+    // c % csz computes the T of chunk c ("owns" it) and pushes it into every CTA's operand ring
+    const uint32_t csz = cluster_nctarank(), rank = cluster_ctarank();
 
     // ---- one-time setup ------------------------------------------------------------------------------------
     if (warp == 0 && lane == 0) {
@@ -190,29 +208,30 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
         for (int i = 0; i < NV; ++i) { mbar_init(&bars[BI.v_full + i], 1); mbar_init(&bars[BI.v_read + i], 4); }
         mbar_init(&bars[BI.x_done], 1); mbar_init(&bars[BI.x_read], 4);
         mbar_init(&bars[BI.r_full], 4); mbar_init(&bars[BI.w_read], 4); mbar_init(&bars[BI.wt_full], 4);
-        for (int i = 0; i < 8; ++i) mbar_init(&bars[BI.row_ready + i], 1);
+        for (int i = 0; i < 4; ++i) mbar_init(&bars[BI.row_ready + i], 1);
+        mbar_init(&bars[BI.g_done], 1); mbar_init(&bars[BI.kg_full], 1); mbar_init(&bars[BI.t_ack], csz);
         for (int i = 0; i < 2; ++i) {
             mbar_init(&bars[BI.s_full + i], 4);
-            mbar_init(&bars[BI.g_done + i], 1); mbar_init(&bars[BI.g_read + i], 4);
+            mbar_init(&bars[BI.t_free + i], csz);
             mbar_init(&bars[BI.p_done + i], 1); mbar_init(&bars[BI.a_full + i], 4);
             mbar_init(&bars[BI.y_done + i], 1); mbar_init(&bars[BI.y_free + i], 4);
-            mbar_init(&bars[BI.t_full + i], 4);
+            mbar_init(&bars[BI.t_full + i], 1);
             mbar_init(&bars[BI.w_done + i], 1);
             mbar_init(&bars[BI.wv_full + i], 4);
             mbar_init(&bars[BI.o2_done + i], 1); mbar_init(&bars[BI.o2_free + i], 4);
             mbar_init(&bars[BI.u_done + i], 1); mbar_init(&bars[BI.u_empty + i], 4);
-            mbar_init(&bars[BI.g_full + i], 1); mbar_init(&bars[BI.g_empty + i], 24);
+            mbar_init(&bars[BI.g_full + i], 1); mbar_init(&bars[BI.g_empty + i], 16);
         }
         fence_mbar_init();
         tma_prefetch_desc(&tq); tma_prefetch_desc(&tk); tma_prefetch_desc(&tv);
     }
     if (warp == 2) tmem_alloc(tmem_slot, L::tmem_cols);
-    // the T operand buffers: the blocks above the diagonal are never written, so they are zeroed once
-    for (uint32_t i = threadIdx.x; i < 2 * L::t_bytes / 16; i += L::kThreads)
-        reinterpret_cast<uint4*>(sm + L::t_off)[i] = make_uint4(0, 0, 0, 0);
+    // the T staging buffer: the blocks above the diagonal are never written, so they are zeroed once
+    for (uint32_t i = threadIdx.x; i < L::t_bytes / 16; i += L::kThreads)
+        reinterpret_cast<uint4*>(sm + L::tstage_off)[i] = make_uint4(0, 0, 0, 0);
     fence_proxy_async_smem();
     tc_fence_before_sync();
-    __syncthreads();
+    cluster_sync();   // every CTA's barriers are initialised before a peer copies a T into it or arrives on them
     tc_fence_after_sync();
     const uint32_t tb = __shfl_sync(0xffffffffu, *tmem_slot, 0);
     GPROF_DECL
@@ -304,22 +323,14 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             if (lane == 0) mbar_arrive(&bars[BI.g_full + slot]);
         }
     } else if (warp == 2) {
-        // ================= issuer: G = K K^T, P = Q K^T =================
+        // ================= issuer: P = Q K^T  (G = K K^T is issued by the T warps, for the chunks this CTA inverts) =================
         constexpr uint32_t idPG = idesc_bf16(kGC, kGC, 0, 0);
         const uint64_t dQ0 = smem_desc(sm_a + L::stage_off, 16, 1024, kSwz128);
         const uint64_t dK0 = smem_desc(sm_a + L::stage_off + L::q_bytes, 16, 1024, kSwz128);
         for (uint32_t c = 0; c < n_chunks; ++c) {
             const uint32_t s = c % NS, pb = c & 1;
             GW_(0, mbar_wait_relaxed(&bars[BI.full + s], (c / NS) & 1));
-            if (c >= 2) GW_(1, mbar_wait_relaxed(&bars[BI.g_read + pb], ((c - 2) >> 1) & 1));             // the T warps have read G(c - 2)
-            tc_fence_after_sync();
             const uint64_t dQ = smem_desc_advance(dQ0, s * L::stage_bytes), dK = smem_desc_advance(dK0, s * L::stage_bytes);
-#pragma unroll 1
-            for (int ks = 0; ks < DK / 16; ++ks) {
-                const uint32_t adv = (ks / 4) * L::half_bytes + (ks % 4) * 32;
-                mma_bf16_ss_w(tb + L::tm_g + pb * kGC, smem_desc_advance(dK, adv), smem_desc_advance(dK, adv), idPG, ks > 0);
-            }
-            mma_commit_w(&bars[BI.g_done + pb]);
             if (c >= 2) GW_(2, mbar_wait_relaxed(&bars[BI.o2_done + pb], ((c - 2) >> 1) & 1));           // O2(c - 2) has read A^q from buffer pb
             tc_fence_after_sync();
 #pragma unroll 1
@@ -348,6 +359,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
         const uint64_t dW0 = smem_desc(sm_a + L::wv_off, 128, L::op_sbo, kSwzNone);
         for (uint32_t c = 0; c < n_chunks; ++c) {
             const uint32_t s = c % NS, sb = c & 1;
+            if (lane == 0) mbar_arrive_expect_tx(&bars[BI.t_full + sb], L::t_bytes);   // T(c): pushed by CTA c % csz (bulk copy into slot sb)
             GW_(0, mbar_wait(&bars[BI.full + s], (c / NS) & 1));
             if (c >= 1) GW_(1, mbar_wait(&bars[BI.x_read], (c - 1) & 1));
             GW_(2, mbar_wait(&bars[BI.s_full + sb], (c >> 1) & 1));
@@ -368,7 +380,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             mma_commit_w(&bars[BI.y_done + sb]);
             // Wm = T R
             GW_(4, mbar_wait(&bars[BI.t_full + sb], (c >> 1) & 1));
-            if (c >= 1) GW_(4, mbar_wait(&bars[BI.w_read], (c - 1) & 1));
+            if (c >= 1) GW_(1, mbar_wait(&bars[BI.w_read], (c - 1) & 1));
             GW_(5, mbar_wait(&bars[BI.r_full], c & 1));
             tc_fence_after_sync();
             const uint64_t dT = smem_desc_advance(dT0, sb * L::t_bytes);
@@ -405,18 +417,37 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
                 mma_commit_w(&bars[BI.o2_done + sb]);
             }
         }
-    } else if (warp >= 4 && warp < 12) {
+    } else if (warp == 4) {
+        // ================= ack warp: tells the owners of T(c + 2) and T(c) that this CTA's Wm(c) has read its copy of T(c) =================
+        // (a remote arrive costs its thread ~1000 cycles: on a warp of its own it is off every other role's path)
+        for (uint32_t c = 0; c < n_chunks; ++c) {
+            const uint32_t sb = c & 1;
+            GW_(0, mbar_wait_relaxed(&bars[BI.w_done + sb], (c >> 1) & 1));
+            if (lane == 0) {
+                if (c + 2 < n_chunks) mbar_arrive_cluster_relaxed(mapa(smem_u32(&bars[BI.t_free + sb]), (c + 2) % csz));   // slot sb is free for T(c + 2)
+                mbar_arrive_cluster_relaxed(mapa(smem_u32(&bars[BI.t_ack]), c % csz));                                       // the owner's staging copy has landed
+            }
+            __syncwarp();
+        }
+    } else if (warp >= 8 && warp < 12) {
         // ================= T warps: A^k = beta_i D_ij G_ij (j < i), T = (I + A^k)^-1 -> MN-major A operand =================
-        // One 64 x 64 bf16 staging matrix per chunk parity (hi and lo terms, row-major, padded rows) holds the blocks of A^k below
-        // the diagonal and the blocks of U = T^T on and above it: warp I writes block row I of both and reads the A^k blocks and
-        // the diagonal blocks of the rows below it, row by row as they become ready (one mbarrier per row: no barrier between the
-        // four warps, whose loads are complementary: row 3 has the most A^k to form, row 0 the most products).  The loops over
-        // blocks are rolled on purpose (the first version unrolled them: 84 KB of SASS per kernel, every role starved by
-        // instruction-cache misses, r02 ncu: 5.5 warps stalled on "no instruction" per issue).
+        // T depends on k, beta and the decays only: the same matrix in every d_v slice of a head.  The slices of a head are a
+        // cluster; CTA c % csz computes T(c) — these four warps, one chunk in csz, far ahead of the carry chain — into a staging
+        // buffer and pushes it into operand slot c % 2 of EVERY CTA of the cluster (bulk copies over distributed shared memory,
+        // completion as transaction bytes on each CTA's t_full barrier).  (The first r02 version computed every T in every CTA:
+        // two sets of four warps, and the chain still waited ~800 cycles per chunk for them.)  The pipeline of an owned chunk is
+        // self-contained: own gate values (the gate warp's ring only runs a few chunks ahead of the chain), own TMA load of the K
+        // tile (into the staging matrix, which is free until A^k is formed), G = K K^T issued by warp 8.
+        // One 64 x 64 bf16 staging matrix (hi and lo terms, row-major, padded rows) holds the blocks of A^k below the diagonal
+        // and the blocks of U = T^T on and above it: warp I writes block row I of both and reads the A^k blocks and the
+        // diagonal blocks of the rows below it, row by row as they become ready (one mbarrier per row).  The loops over blocks are
+        // rolled on purpose (the first version unrolled them: 84 KB of SASS per kernel, every role starved by instruction-cache
+        // misses, r02 ncu: 5.5 warps stalled on "no instruction" per issue).
         const int I = q;                                   // block row of A^k this warp forms = block row of U it fills
         const int ia = 16 * I + g8, ib = ia + 8;
-        const uint32_t tset = warp < 8 ? 1u : 0u;          // warps 8-11 take the even chunks, warps 4-7 the odd ones
-        float* lt = reinterpret_cast<float*>(sm + L::lt_off) + (tset * 4 + I) * 16 * L::lt_pitch;   // fp32 diagonal block, transposed: lt[j][i]
+        float* lt = reinterpret_cast<float*>(sm + L::lt_off) + I * 16 * L::lt_pitch;   // fp32 diagonal block, transposed: lt[j][i]
+        float* b2 = reinterpret_cast<float*>(sm + L::tg_off) + I * 2 * kGC;           // this warp's copy of the chunk's gate values
+        float* be = b2 + kGC;
         const uint32_t mi = lane >> 3, rr = lane & 7;
         // ldmatrix row addresses inside a 16 x 16 block, by the order of the four 8 x 8 matrices:
         //   "rc": (rows 0-7, cols 0-7), (rows 8-15, cols 0-7), (rows 0-7, cols 8-15), (rows 8-15, cols 8-15)
@@ -424,24 +455,82 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
         const uint32_t rc_lane = (rr + 8 * (mi & 1)) * L::a_pitch + 16 * (mi >> 1);
         const uint32_t cr_lane = (rr + 8 * (mi >> 1)) * L::a_pitch + 16 * (mi & 1);
         auto blk = [](int r, int cc) { return (uint32_t)((16 * r) * L::a_pitch + (16 * cc) * 2); };
-        for (uint32_t c = tset; c < n_chunks; c += 2) {
-            const uint32_t tbuf = tset, bt = c / kGCPB, gslot = bt & 1;
-            GW_(0, mbar_wait_relaxed(&bars[BI.g_full + gslot], (bt >> 1) & 1));   // (every chunk: a wait on a completed phase returns at once)
-            const float* b2 = gate + gslot * 3 * kGBatch + (c % kGCPB) * kGC;
-            const float* be = b2 + 2 * kGBatch;
-            const float bia = b2[ia], bib = b2[ib], bea = be[ia], beb = be[ib];
-            // T operand buffer tbuf is free once Wm(c - 2) has completed; Wm(c - 2) needed the whole of T(c - 2), so every T warp is
-            // also done with staging matrix tbuf
-            if (c >= 2) GW_(2, mbar_wait_relaxed(&bars[BI.w_done + tbuf], ((c - 2) >> 1) & 1));
-            uint8_t* ast = sm + L::a_off + tbuf * 2 * L::a_term_bytes;
-            const uint32_t a_hi = sm_a + L::a_off + tbuf * 2 * L::a_term_bytes, a_lo = a_hi + L::a_term_bytes;
-            uint8_t* tbase = sm + L::t_off + tbuf * L::t_bytes;
-            GW_(1, mbar_wait_relaxed(&bars[BI.g_done + tbuf], (c >> 1) & 1));
-            tc_fence_after_sync();
+        uint8_t* ast = sm + L::a_off;
+        const uint32_t a_hi = sm_a + L::a_off, a_lo = a_hi + L::a_term_bytes;
+        uint8_t* tbase = sm + L::tstage_off;
+        constexpr uint32_t idG = idesc_bf16(kGC, kGC, 0, 0);
+        const uint64_t dKg = smem_desc(sm_a + L::a_off, 16, 1024, kSwz128);
+        uint32_t k_own = 0;                                // owned chunks done: the phase of this pipeline's own barriers
+        // raw a / beta of owned chunk number k (chunk cc) -> traw[k & 1], by warp 8: asynchronous copies, waited for before the
+        // barrier that ends the preceding owned chunk.  Tokens beyond T: a = 1, beta = 0 (identity).
+        auto load_raw = [&](uint32_t cc, uint32_t k) {
+            float* raw = reinterpret_cast<float*>(sm + L::traw_off) + (k & 1) * 2 * kGC;
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const uint64_t tt = (uint64_t)cc * kGC + lane + 32 * u;
+                if (tt < T) {
+                    const size_t idx = ((size_t)b * t_stride + tt) * H + h;
+                    cp_async_4(raw + lane + 32 * u, g + idx);
+                    cp_async_4(raw + kGC + lane + 32 * u, beta + idx);
+                } else {
+                    raw[lane + 32 * u] = 1.f;
+                    raw[kGC + lane + 32 * u] = 0.f;
+                }
+            }
+            cp_async_commit();
+        };
+        if (rank < n_chunks) {
+            if (I == 0) {
+                load_raw(rank, 0);
+                cp_async_wait_all();
+            }
+            named_bar_sync(1, 128);
+        }
+        for (uint32_t c = rank; c < n_chunks; c += csz, ++k_own) {
             GSEG_START
+            if (I == 0 && c + csz < n_chunks) load_raw(c + csz, k_own + 1);
+            if (I == 0 && lane == 0) {   // the K tile of the chunk (everybody is past the previous chunk's staging matrix: barrier below)
+                mbar_arrive_expect_tx(&bars[BI.kg_full], L::q_bytes);
+                tma_load_5d(sm + L::a_off, &tk, &bars[BI.kg_full], 0, (int)(c * kGC), 0, (int)h, (int)b);
+            }
+            // gate values of the chunk from the raw a / beta that warp 8 copied in one owned chunk ahead (cp.async): lane l owns
+            // tokens 2 l, 2 l + 1, then a warp scan.  (Each of the four warps keeps its own copy: no barrier.  The summation order
+            // differs from the gate warp's, so these b agree with the chain's to an ulp of the exponent, not bit for bit; both are
+            // functions of the chunk's inputs only.)
+            {
+                const float* raw = reinterpret_cast<const float*>(sm + L::traw_off) + (k_own & 1) * 2 * kGC;
+                const float2 gv = *reinterpret_cast<const float2*>(raw + 2 * lane);
+                const float2 bv = *reinterpret_cast<const float2*>(raw + kGC + 2 * lane);
+                const float l0 = log2f(gv.x), l1 = l0 + log2f(gv.y);
+                float incl = l1;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const float up = __shfl_up_sync(0xffffffffu, incl, d);
+                    if (lane >= d) incl += up;
+                }
+                const float excl = incl - l1;
+                *reinterpret_cast<float2*>(b2 + 2 * lane) = make_float2(excl + l0, excl + l1);
+                *reinterpret_cast<float2*>(be + 2 * lane) = bv;
+                __syncwarp();
+            }
+            const float bia = b2[ia], bib = b2[ib], bea = be[ia], beb = be[ib];
+            GSEG(0);
+            if (I == 0) {   // G = K K^T
+                mbar_wait_relaxed(&bars[BI.kg_full], k_own & 1);
+                tc_fence_after_sync();
+#pragma unroll 1
+                for (int ks = 0; ks < DK / 16; ++ks) {
+                    const uint32_t adv = (ks / 4) * L::half_bytes + (ks % 4) * 32;
+                    mma_bf16_ss_w(tb + L::tm_g, smem_desc_advance(dKg, adv), smem_desc_advance(dKg, adv), idG, ks > 0);
+                }
+                mma_commit_w(&bars[BI.g_done]);
+            }
+            mbar_wait_relaxed(&bars[BI.g_done], k_own & 1);   // (the MMAs have also finished reading the K tile: the staging matrix is free)
+            tc_fence_after_sync();
+            GSEG(1);
             uint32_t cur[8], nxt[8];
-            tmem_ld_16x256b_x2(tmem_addr(tb, 32 * q, L::tm_g + tbuf * kGC + 16 * I), cur);
-            if (I > 0) tmem_ld_16x256b_x2(tmem_addr(tb, 32 * q, L::tm_g + tbuf * kGC), nxt);
+            tmem_ld_16x256b_x2(tmem_addr(tb, 32 * q, L::tm_g + 16 * I), cur);
+            if (I > 0) tmem_ld_16x256b_x2(tmem_addr(tb, 32 * q, L::tm_g), nxt);
             tmem_ld_wait();
             // the diagonal block in fp32, transposed and masked (j < i), for the substitution
 #pragma unroll
@@ -466,7 +555,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             for (int m2 = 0; m2 < I; ++m2) {
 #pragma unroll
                 for (int i = 0; i < 8; ++i) cur[i] = nxt[i];
-                if (m2 + 1 < I) tmem_ld_16x256b_x2(tmem_addr(tb, 32 * q, L::tm_g + tbuf * kGC + 16 * (m2 + 1)), nxt);
+                if (m2 + 1 < I) tmem_ld_16x256b_x2(tmem_addr(tb, 32 * q, L::tm_g + 16 * (m2 + 1)), nxt);
 #pragma unroll
                 for (int jb = 0; jb < 2; ++jb) {
                     const int j0 = 16 * m2 + 8 * jb + 2 * t4;
@@ -486,8 +575,6 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
                 tmem_ld_wait();
             }
             tc_fence_before_sync();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&bars[BI.g_read + tbuf]);
             GSEG(3);
             // T_II = (I + A_II)^-1, column by column: lane col solves (I + A_II) x = e_col by forward substitution in fp32
             // (right-looking: once x_j is final every later row takes its term; independent FMAs, the dependency chain is one FMA
@@ -513,6 +600,10 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
                 uint32_t hi[8], lo[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) hi[e] = split2(x[2 * e], x[2 * e + 1], lo[e]);
+                // the T staging buffer still holds T(c - csz): it may be rewritten once every CTA's copy of it has landed (t_ack: every
+                // CTA's Wm(c - csz) has completed).  Waited for here, at the first write, not at the top: the push, the peers' Wm and
+                // their acknowledgement take ~4000 cycles, which the gate values, the K tile, G, A^k and the substitution overlap.
+                if (k_own >= 1) mbar_wait_relaxed(&bars[BI.t_ack], (k_own - 1) & 1);
                 if (lane < 16) {
                     uint8_t* dh = ast + blk(I, I) + col * L::a_pitch;   // U_II row-major in the staging matrix
                     *reinterpret_cast<uint4*>(dh) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
@@ -529,13 +620,13 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(&bars[BI.row_ready + 4 * tbuf + I]);   // block row I of A^k and U_II are staged
+            if (lane == 0) mbar_arrive(&bars[BI.row_ready + I]);   // block row I of A^k and U_II are staged
             GSEG(4);
             // block row I of U = T^T:  U_I,Ic = -(sum_{K=I}^{Ic-1} U_I,K (A^k_{Ic,K})^T) U_Ic,Ic.  (The three hi / lo terms of a
             // product accumulate in place: separate accumulators shorten the mma chain but cost more instructions than they save.)
 #pragma unroll 1
             for (int Ic = I + 1; Ic < 4; ++Ic) {
-                GW_(5, mbar_wait(&bars[BI.row_ready + 4 * tbuf + Ic], (c >> 1) & 1));   // (a ring of two: the writer may be a chunk ahead)
+                mbar_wait(&bars[BI.row_ready + Ic], k_own & 1);
                 float z[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
 #pragma unroll 1
                 for (int K = I; K < Ic; ++K) {
@@ -584,12 +675,20 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
                 __syncwarp();
             }
             GSEG(6);
-            fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0) {
-                mbar_arrive(&bars[BI.t_full + tbuf]);
-                if ((c % kGCPB) >= (uint32_t)kGCPB - 2 || c + 2 >= n_chunks) mbar_arrive(&bars[BI.g_empty + gslot]);   // this set's last chunk of the batch
+            fence_proxy_async_smem();       // this warp's part of T: generic-proxy writes -> visible to the bulk copies
+            tc_fence_before_sync();         // (and its reads of G are ordered before the next chunk's G MMAs)
+            if (I == 0) cp_async_wait_all();   // the next owned chunk's raw gate values have landed
+            named_bar_sync(1, 128);         // all of T(c) is in the staging buffer; G and the staging matrix may be reused
+            GSEG(5);
+            if (I == 0 && lane == 0) {
+                // slot c % 2 of every CTA is free once every CTA's Wm(c - 2) has completed.  Arrivals on this CTA's t_free come for the
+                // chunks it owns only (all of the same parity: csz is even), one phase per owned chunk c >= 2.
+                if (c >= 2) mbar_wait(&bars[BI.t_free + (c & 1)], (k_own - (rank < 2 ? 1u : 0u)) & 1);
+                const uint32_t dst = sm_a + L::t_off + (c & 1) * L::t_bytes, full = smem_u32(&bars[BI.t_full + (c & 1)]);
+                for (uint32_t pr = 0; pr < csz; ++pr) bulk_copy_to_cluster(mapa(dst, pr), sm_a + L::tstage_off, L::t_bytes, mapa(full, pr));
             }
+            __syncwarp();
+            GSEG(2);
         }
     } else if (warp >= 12 && warp < 16) {
         // ================= R / W warps: R = beta (V - Gamma X) -> operand;  Wm -> [Wm_hi | Wm_lo] and W~ operands =================
@@ -888,7 +987,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
     // ---- teardown: the state and epilogue warps have waited on the last commits of every MMA group but G / P, whose results the
     // T and score warps have read ----
     tc_fence_before_sync();
-    __syncthreads();
+    cluster_sync();   // no peer still copies into this CTA or arrives on its barriers
     if (warp == 2) tmem_dealloc(tb, L::tmem_cols);
 }
 
@@ -907,9 +1006,20 @@ static int launch_gdn_t(esc_ctx* ctx, const ScanShape& s, const void* q, const v
     if (rc == ESC_OK) rc = make_tmap_halves(&tk, kk, DK, s.H, T, ts, s.B, kGC);
     if (rc == ESC_OK) rc = make_tmap(&tv, vv, s.dv, s.H, T, ts, s.B, kGW, kGC, CU_TENSOR_MAP_SWIZZLE_32B);
     if (rc != ESC_OK) return rc;
-    dim3 grid(s.dv / kGW, s.B * s.H);
-    esc_gdn_scan_kernel<DK><<<grid, L::kThreads, L::total, stream>>>(tq, tk, tv, g, beta, state_in, state_out, o, s.H, s.dv, T, t_stride);
-    ESC_CUDA(cudaGetLastError());
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(s.dv / kGW, s.B * s.H);   // the d_v slices of a (b, h) are one cluster (4 or 8 CTAs): they share the chunk inverses
+    cfg.blockDim = dim3(L::kThreads);
+    cfg.dynamicSmemBytes = L::total;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    memset(attr, 0, sizeof attr);
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = kGdnCluster;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ESC_CUDA(cudaLaunchKernelEx(&cfg, esc_gdn_scan_kernel<DK>, tq, tk, tv, g, beta, state_in, state_out, o, s.H, s.dv, T, t_stride));
     return ESC_OK;
 }
 
@@ -919,7 +1029,7 @@ extern "C" int esc_debug_gdn_prof_read(long long* host) { return (int)cudaMemcpy
 
 int launch_gdn_mma(esc_ctx* ctx, const ScanShape& s, const void* q, const void* k, const void* v, const float* g, const float* beta,
                    const float* state_in, float* state_out, float* o, uint64_t T, uint64_t t_stride, cudaStream_t stream) {
-    if (s.dv % kGW) return ESC_ERR_UNSUPPORTED;
+    if (s.dv % kGW || (s.dv / kGW) % kGdnCluster) return ESC_ERR_UNSUPPORTED;
     if (s.dk == 128) return launch_gdn_t<128>(ctx, s, q, k, v, g, beta, state_in, state_out, o, T, t_stride, stream);
     if (s.dk == 64) return launch_gdn_t<64>(ctx, s, q, k, v, g, beta, state_in, state_out, o, T, t_stride, stream);
     return ESC_ERR_UNSUPPORTED;
