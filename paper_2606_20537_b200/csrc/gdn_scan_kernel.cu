@@ -479,8 +479,15 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             }
             cp_async_commit();
         };
+        // the K tile of an owned chunk -> the staging matrix (free from the barrier that ends the preceding owned chunk until A^k is
+        // formed); issued right after that barrier, so that the load flies during the push and the gate values
+        auto load_k = [&](uint32_t cc) {
+            mbar_arrive_expect_tx(&bars[BI.kg_full], L::q_bytes);
+            tma_load_5d(sm + L::a_off, &tk, &bars[BI.kg_full], 0, (int)(cc * kGC), 0, (int)h, (int)b);
+        };
         if (rank < n_chunks) {
             if (I == 0) {
+                if (lane == 0) load_k(rank);
                 load_raw(rank, 0);
                 cp_async_wait_all();
             }
@@ -489,10 +496,6 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
         for (uint32_t c = rank; c < n_chunks; c += csz, ++k_own) {
             GSEG_START
             if (I == 0 && c + csz < n_chunks) load_raw(c + csz, k_own + 1);
-            if (I == 0 && lane == 0) {   // the K tile of the chunk (everybody is past the previous chunk's staging matrix: barrier below)
-                mbar_arrive_expect_tx(&bars[BI.kg_full], L::q_bytes);
-                tma_load_5d(sm + L::a_off, &tk, &bars[BI.kg_full], 0, (int)(c * kGC), 0, (int)h, (int)b);
-            }
             // gate values of the chunk from the raw a / beta that warp 8 copied in one owned chunk ahead (cp.async): lane l owns
             // tokens 2 l, 2 l + 1, then a warp scan.  (Each of the four warps keeps its own copy: no barrier.  The summation order
             // differs from the gate warp's, so these b agree with the chain's to an ulp of the exponent, not bit for bit; both are
@@ -681,6 +684,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             named_bar_sync(1, 128);         // all of T(c) is in the staging buffer; G and the staging matrix may be reused
             GSEG(5);
             if (I == 0 && lane == 0) {
+                if (c + csz < n_chunks) load_k(c + csz);
                 // slot c % 2 of every CTA is free once every CTA's Wm(c - 2) has completed.  Arrivals on this CTA's t_free come for the
                 // chunks it owns only (all of the same parity: csz is even), one phase per owned chunk c >= 2.
                 if (c >= 2) mbar_wait(&bars[BI.t_free + (c & 1)], (k_own - (rank < 2 ? 1u : 0u)) & 1);
