@@ -134,7 +134,7 @@ struct GdnCfg {
 };
 
 struct GdnBars {
-    int full, empty, v_full, v_read, s_full, g_done, kg_full, t_free, t_ack, p_done, a_full, x_done, x_read, y_done, y_free, t_full, r_full, w_done,
+    int full, empty, v_full, v_read, s_full, g_done, kg_full, t_free, t_ack, t_staged, p_done, a_full, x_done, x_read, y_done, y_free, t_full, r_full, w_done,
         w_read, wv_full, wt_full, o2_done, o2_free, u_done, u_empty, g_full, g_empty, row_ready, count;
 };
 template <int DK>
@@ -151,6 +151,7 @@ __device__ __forceinline__ constexpr GdnBars gdn_bars() {
     b.kg_full = i; i += 1;
     b.t_free = i; i += 2;
     b.t_ack = i; i += 1;
+    b.t_staged = i; i += 1;
     b.p_done = i; i += 2;
     b.a_full = i; i += 2;
     b.x_done = i; i += 1;
@@ -209,7 +210,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
         mbar_init(&bars[BI.x_done], 1); mbar_init(&bars[BI.x_read], 4);
         mbar_init(&bars[BI.r_full], 4); mbar_init(&bars[BI.w_read], 4); mbar_init(&bars[BI.wt_full], 4);
         for (int i = 0; i < 4; ++i) mbar_init(&bars[BI.row_ready + i], 1);
-        mbar_init(&bars[BI.g_done], 1); mbar_init(&bars[BI.kg_full], 1); mbar_init(&bars[BI.t_ack], csz);
+        mbar_init(&bars[BI.g_done], 1); mbar_init(&bars[BI.kg_full], 1); mbar_init(&bars[BI.t_ack], csz); mbar_init(&bars[BI.t_staged], 1);
         for (int i = 0; i < 2; ++i) {
             mbar_init(&bars[BI.s_full + i], 4);
             mbar_init(&bars[BI.t_free + i], csz);
@@ -426,6 +427,21 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             if (lane == 0) {
                 if (c + 2 < n_chunks) mbar_arrive_cluster_relaxed(mapa(smem_u32(&bars[BI.t_free + sb]), (c + 2) % csz));   // slot sb is free for T(c + 2)
                 mbar_arrive_cluster_relaxed(mapa(smem_u32(&bars[BI.t_ack]), c % csz));                                       // the owner's staging copy has landed
+            }
+            __syncwarp();
+        }
+    } else if (warp == 5) {
+        // ================= push warp: T(c) of an owned chunk, staged by the T warps -> slot c % 2 of every CTA of the cluster =================
+        // Slot c % 2 of every CTA is free once every CTA's Wm(c - 2) has completed.  Arrivals on this CTA's t_free come for the chunks it
+        // owns only (all of the same parity: csz is even), one phase per owned chunk c >= 2.  (On a warp of its own: the T warps
+        // are typically a few chunks ahead of the chain, and waiting for the slot would hold up their next chunk.)
+        uint32_t k_own = 0;
+        for (uint32_t c = rank; c < n_chunks; c += csz, ++k_own) {
+            GW_(0, mbar_wait_relaxed(&bars[BI.t_staged], k_own & 1));
+            if (c >= 2) GW_(1, mbar_wait_relaxed(&bars[BI.t_free + (c & 1)], (k_own - (rank < 2 ? 1u : 0u)) & 1));
+            if (lane == 0) {
+                const uint32_t dst = sm_a + L::t_off + (c & 1) * L::t_bytes, full = smem_u32(&bars[BI.t_full + (c & 1)]);
+                for (uint32_t pr = 0; pr < csz; ++pr) bulk_copy_to_cluster(mapa(dst, pr), sm_a + L::tstage_off, L::t_bytes, mapa(full, pr));
             }
             __syncwarp();
         }
@@ -685,11 +701,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             GSEG(5);
             if (I == 0 && lane == 0) {
                 if (c + csz < n_chunks) load_k(c + csz);
-                // slot c % 2 of every CTA is free once every CTA's Wm(c - 2) has completed.  Arrivals on this CTA's t_free come for the
-                // chunks it owns only (all of the same parity: csz is even), one phase per owned chunk c >= 2.
-                if (c >= 2) mbar_wait(&bars[BI.t_free + (c & 1)], (k_own - (rank < 2 ? 1u : 0u)) & 1);
-                const uint32_t dst = sm_a + L::t_off + (c & 1) * L::t_bytes, full = smem_u32(&bars[BI.t_full + (c & 1)]);
-                for (uint32_t pr = 0; pr < csz; ++pr) bulk_copy_to_cluster(mapa(dst, pr), sm_a + L::tstage_off, L::t_bytes, mapa(full, pr));
+                mbar_arrive(&bars[BI.t_staged]);   // the push warp takes it from here: these warps go on with the next owned chunk
             }
             __syncwarp();
             GSEG(2);
