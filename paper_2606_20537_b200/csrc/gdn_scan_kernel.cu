@@ -4,7 +4,7 @@
 //
 // Per chunk of C = 64 tokens, S the state at the chunk's start, b_i = sum_{r<=i} log2 a_r (inclusive, inside the chunk),
 // D_ij = 2^(b_i - b_j) (<= 1 for j <= i), Gamma = diag(2^(b_i)), w_i = beta_i (v_i - u_i) the rows the 64 rank-one updates add:
-//     G = K K^T , P = Q K^T                                   (64 x 64)    tcgen05.mma  M=64 N=64 K=d_k   (SS)
+//     G = K K^T , P = Q K^T                                   (64 x 64)    tcgen05.mma  M=64 N=64 K=d_k   (SS); G in the owning CTA only
 //     A^k_ij = beta_i D_ij G_ij  (j <  i) ,  T = (I + A^k)^-1  (64 x 64)    fp32 ALU + warp-level MMAs, OFF the carry chain
 //     A^q_ij =        D_ij P_ij  (j <= i)                      (64 x 64)    in place in TMEM (bf16 hi | lo), as in scan_kernel.cu
 //     [X | Y] = [K ; Q] [S_hi | S_lo]                          (64 x 2W)    tcgen05.mma  M=64 N=2W K=d_k   (SS), W = 16 columns
@@ -18,21 +18,29 @@
 //
 // Decomposition: the columns of S are independent, one CTA owns (b, h, 16 columns of d_v) and walks the chunks in order with its
 // [d_k x 16] state slice in registers.  The carry chain of a chunk is  S -> X (MMA) -> R (registers) -> Wm (MMA) -> W~
-// (registers) -> U (MMA) -> S: three small MMA groups and three register passes; everything else (G, P, the inverse T, the
-// scores, Y, the outputs) is computed beside it by warps of its own and meets the chain through mbarriers.
+// (registers) -> U (MMA) -> S: three small MMA groups and three register passes; everything else (P, the scores, Y, the
+// outputs) is computed beside it by warps of its own and meets the chain through mbarriers.
 //
-// The inverse T.  (I + A^k) is unit lower triangular, 4 x 4 blocks of 16 x 16.  Each of four warps inverts one diagonal block in
-// fp32 (one column per lane, forward substitution), then warp J fills block COLUMN J of T by the block recursion
+// The inverse T is shared.  T = (I + A^k)^-1 depends on k, beta and the decays only: it is the same matrix in every d_v slice of a
+// head.  Four slices form a thread-block cluster, and CTA c % 4 computes T(c) for all of them ("owns" chunk c): its four T warps
+// work on one chunk in four, several chunks ahead of the carry chain, with a pipeline of their own (their own gate values, their
+// own TMA load of the K tile, G = K K^T issued by themselves), stage the result in shared memory, and a push warp copies it
+// into operand slot c % 2 of EVERY CTA of the cluster (cp.async.bulk over distributed shared memory, completion as transaction
+// bytes on each CTA's t_full barrier).  Flow control is two remote arrivals per chunk and CTA, from a warp of its own ("my
+// Wm(c) has read its copy": the slot is free for T(c + 2), and the owner's staging buffer for its next chunk).
+// (I + A^k) is unit lower triangular, 4 x 4 blocks of 16 x 16: each T warp inverts one diagonal block in fp32 (one column per
+// lane, forward substitution), then warp J fills block COLUMN J of T by the block recursion
 //     T_IJ = - T_II  sum_{K=J}^{I-1} A^k_IK T_KJ      evaluated on the transpose, U = T^T:  U_JI = -(sum_K U_JK (A^k_IK)^T) U_II,
-// where the running blocks U_JK are A operands of the next product (an accumulator fragment re-read as an A fragment: no data
-// movement).  These 16 x 16 x 16 products run as warp-level mma.sync (two-term bf16 splits, three products per term pair): 16
-// block products per chunk, far from the 64 x 64 x d_k contractions above, and a tcgen05 round trip through TMEM per block
-// product (six deep) would not fit beside the chain.  T lands in shared memory as the MN-major A operand of Wm = T R.
+// where the running blocks U_JK are A operands of the next product.  These 16 x 16 x 16 products run as warp-level mma.sync
+// (two-term bf16 splits): the only mma.sync in the library, 96 instructions per owned chunk.  The same products in fp32 on the
+// CUDA cores (packed FFMA2, two levels of 2 x 2 block inverses, no mma.sync at all) are bit-for-bit as good and were measured
+// at 0.410 ms against 0.395 ms for 16 448 tokens: their instruction stream competes with the chain's warps for issue slots.
 //
 // Warp roles (28 warps, mbarrier pipeline, no CTA-wide barrier in the loop):
 //   warp 0       TMA producer (Q, K whole tiles through the 5-D halves map, V tile; L2 prefetch ahead)
 //   warp 1       gate warp: b = prefix sums of log2 a, 2^b, beta, 256 tokens per batch
-//   warp 2       issuer of G and P            warp 3   issuer of the chain: X, Y, Wm, U            warp 4   issuer of O2
+//   warp 2       issuer of P                  warp 3   issuer of the chain (X, Y, Wm, U) and of O2
+//   warp 4       ack warp (remote arrivals)   warp 5   push warp (T of an owned chunk -> the cluster)
 //   warps 8-11   T warps (the inverse)        warps 12-15  R / W warps (the register passes of the chain)
 //   warps 16-19  score warps (A^q in TMEM)    warps 20-23  epilogue (o)            warps 24-27  state warps (the carry)
 //
@@ -55,9 +63,6 @@ constexpr int kGC = 64;            // tokens per chunk
 constexpr int kGW = 16;            // d_v columns per CTA
 constexpr int kGBatch = 256;       // tokens per gate batch
 constexpr int kGCPB = kGBatch / kGC;
-#ifndef ESC_GDN_NS
-#define ESC_GDN_NS 3
-#endif
 #ifndef ESC_GDN_CLUSTER
 #define ESC_GDN_CLUSTER 4
 #endif
@@ -83,7 +88,7 @@ __device__ long long g_gdn_prof[32 * 8];
 template <int DK>
 struct GdnCfg {
     static constexpr int NH = DK / 64;                       // 64-column halves of a Q / K tile
-    static constexpr int NS = ESC_GDN_NS;                    // Q | K stages
+    static constexpr int NS = 3;                             // Q | K stages (2: 4 % slower)
     static constexpr int NV = 4;                             // V tiles
     static constexpr int kWarps = 28;
     static constexpr int kThreads = kWarps * 32;
