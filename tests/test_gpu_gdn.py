@@ -57,6 +57,26 @@ def test_gdn_vs_oracle(esc, ctx, B, H, dk, dv, T, gate, with_s0):
     assert err_o(o.cpu().numpy(), o_ref) <= 5e-5 and err_s(s.cpu().numpy(), s_ref) <= 5e-5   # two-term bf16 operands, fp32 accumulation: far inside the gates
 
 
+@pytest.mark.parametrize("T", [128, 191, 192, 257, 320, 449, 512, 577, 1100])
+@pytest.mark.parametrize("dv", [64, 128])
+def test_gdn_chunk_counts_around_the_cluster_period(esc, ctx, T, dv):
+    """The chunk inverses are computed by the CTAs of a cluster in turn (chunk c by CTA c % 4) and pushed to the others two
+    operand slots deep: chunk counts of 2 ... 18 cover every phase of that rotation, ragged tails included; d_v = 64 is one
+    cluster per head, d_v = 128 two."""
+    B, H, dk = 1, 2, 128
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(75, T, dv), gate="slow")
+    beta = synth.gdn_beta(B, T, H, seed_ids=(75, T, dv))
+    s0 = synth.scan_state(B, H, dk, dv, seed_ids=(76,), scale=0.3)
+    o, s, _ = run_gdn(esc, ctx, scan_dev_inputs(si), to_dev(beta), B, T, H, dk, dv, s0=to_dev(s0))
+    q, k, v, g = si.as_f32()
+    o_ref, s_ref = oracle.gdn_recurrence(q, k, v, g, beta, s0.astype(np.float64))
+    assert err_o(o.cpu().numpy(), o_ref) <= 5e-5 and err_s(s.cpu().numpy(), s_ref) <= 5e-5
+    assert_state_close(s, s_ref)
+    # and the same call twice gives the same bits (no dependence on the arrival order of the pushed inverses)
+    o2, s2, _ = run_gdn(esc, ctx, scan_dev_inputs(si), to_dev(beta), B, T, H, dk, dv, s0=to_dev(s0))
+    assert bits_equal(o, o2) and bits_equal(s, s2)
+
+
 def test_gdn_restore_continue_bit_identical_at_chunk_boundaries(esc, ctx):
     B, H, dk, dv, T = 1, 4, 128, 128, 333
     si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(72,), gate="slow")
