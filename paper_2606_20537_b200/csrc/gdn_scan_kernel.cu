@@ -208,6 +208,9 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
     // c % csz computes the T of chunk c ("owns" it) and pushes it into every CTA's operand ring
     const uint32_t csz = cluster_nctarank(), rank = cluster_ctarank();
 
+    // Programmatic dependent launch: the next kernel of the stream (typically the next layer's scan) may start its on-chip setup
+    // while this one runs; everything this kernel reads from or writes to global memory comes after griddepcontrol.wait below.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // ---- one-time setup ------------------------------------------------------------------------------------
     if (warp == 0 && lane == 0) {
         for (int i = 0; i < NS; ++i) { mbar_init(&bars[BI.full + i], 1); mbar_init(&bars[BI.empty + i], 2); }
@@ -239,6 +242,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
     tc_fence_before_sync();
     cluster_sync();   // every CTA's barriers are initialised before a peer copies a T into it or arrives on them
     tc_fence_after_sync();
+    asm volatile("griddepcontrol.wait;" ::: "memory");   // ---- global memory may be touched from here on ----
     const uint32_t tb = __shfl_sync(0xffffffffu, *tmem_slot, 0);
     GPROF_DECL
 
@@ -1032,14 +1036,16 @@ static int launch_gdn_t(esc_ctx* ctx, const ScanShape& s, const void* q, const v
     cfg.blockDim = dim3(L::kThreads);
     cfg.dynamicSmemBytes = L::total;
     cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     memset(attr, 0, sizeof attr);
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = kGdnCluster;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.* in the kernel
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = 2;
     ESC_CUDA(cudaLaunchKernelEx(&cfg, esc_gdn_scan_kernel<DK>, tq, tk, tv, g, beta, state_in, state_out, o, s.H, s.dv, T, t_stride));
     return ESC_OK;
 }
