@@ -67,6 +67,10 @@ constexpr int kGCPB = kGBatch / kGC;
 #define ESC_GDN_CLUSTER 4
 #endif
 constexpr int kGdnCluster = ESC_GDN_CLUSTER;   // d_v slices of a head that share the chunk inverses (even)
+// Calls of up to kGdnShortT tokens (the suffix after a restore: one chunk) launch WITHOUT the cluster: every CTA inverts its
+// own chunks (the same instructions on the same inputs: same bits) and the push is a local copy; with a single chunk there is
+// nothing to share, and the cluster launch and the distributed-shared-memory hop are on the first chunk's path.
+constexpr uint64_t kGdnShortT = 64;     // (two chunks: 11.3 us without the cluster against 10.9 with it)
 constexpr int kGAhead = 4;         // chunks prefetched into L2 ahead of the shared-memory ring
 
 #ifdef ESC_GDN_PROF   // bring-up only: cycles every role of CTA (0,0) spends in each of its waits / sections, and in its loop in total
@@ -442,12 +446,13 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
     } else if (warp == 5) {
         // ================= push warp: T(c) of an owned chunk, staged by the T warps -> slot c % 2 of every CTA of the cluster =================
         // Slot c % 2 of every CTA is free once every CTA's Wm(c - 2) has completed.  Arrivals on this CTA's t_free come for the chunks it
-        // owns only (all of the same parity: csz is even), one phase per owned chunk c >= 2.  (On a warp of its own: the T warps
+        // owns only (all of the same parity when csz is even; without a cluster, csz = 1, every chunk), one phase per owned chunk c >= 2.  (On a warp of its own: the T warps
         // are typically a few chunks ahead of the chain, and waiting for the slot would hold up their next chunk.)
         uint32_t k_own = 0;
         for (uint32_t c = rank; c < n_chunks; c += csz, ++k_own) {
             GW_(0, mbar_wait_relaxed(&bars[BI.t_staged], k_own & 1));
-            if (c >= 2) GW_(1, mbar_wait_relaxed(&bars[BI.t_free + (c & 1)], (k_own - (rank < 2 ? 1u : 0u)) & 1));
+            // phase of t_free[c % 2] here: the owned chunks before this one that used the slot and had a predecessor (c' >= 2)
+            if (c >= 2) GW_(1, mbar_wait_relaxed(&bars[BI.t_free + (c & 1)], (csz > 1 ? k_own - (rank < 2 ? 1u : 0u) : (c - 2) >> 1) & 1));
             if (lane == 0) {
                 const uint32_t dst = sm_a + L::t_off + (c & 1) * L::t_bytes, full = smem_u32(&bars[BI.t_full + (c & 1)]);
                 for (uint32_t pr = 0; pr < csz; ++pr) bulk_copy_to_cluster(mapa(dst, pr), sm_a + L::tstage_off, L::t_bytes, mapa(full, pr));
@@ -1039,7 +1044,7 @@ static int launch_gdn_t(esc_ctx* ctx, const ScanShape& s, const void* q, const v
     cudaLaunchAttribute attr[2];
     memset(attr, 0, sizeof attr);
     attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = kGdnCluster;
+    attr[0].val.clusterDim.x = T <= kGdnShortT ? 1 : kGdnCluster;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.* in the kernel

@@ -77,6 +77,24 @@ def test_gdn_chunk_counts_around_the_cluster_period(esc, ctx, T, dv):
     assert bits_equal(o, o2) and bits_equal(s, s2)
 
 
+@pytest.mark.parametrize("dk,dv", [(128, 128), (64, 64)])
+def test_gdn_short_call_matches_long_call_prefix_bitwise(esc, ctx, dk, dv):
+    """Calls of up to 64 tokens launch without the cluster (every CTA inverts its own chunk); longer calls share the inverses
+    across four d_v slices.  Same instructions on the same inputs: the first 64 tokens of a long call and a 64-token call give the
+    same o bits, and a chain of 64-token calls ends in the long call's state."""
+    B, H, T = 1, 3, 256
+    si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(77, dk), gate="slow")
+    beta = to_dev(synth.gdn_beta(B, T, H, seed_ids=(77, dk)))
+    s0 = to_dev(synth.scan_state(B, H, dk, dv, seed_ids=(78,), scale=0.3))
+    dev_in = scan_dev_inputs(si)
+    o_long, s_long, _ = run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv, s0=s0)
+    s = s0
+    for t0 in range(0, T, 64):
+        o_b, s, _ = run_gdn(esc, ctx, dev_in, beta, B, T, H, dk, dv, s0=s, t0=t0, n=64)
+        assert bits_equal(o_b, o_long[:, t0:t0 + 64]), t0
+    assert bits_equal(s, s_long)
+
+
 def test_gdn_restore_continue_bit_identical_at_chunk_boundaries(esc, ctx):
     B, H, dk, dv, T = 1, 4, 128, 128, 333
     si = synth.scan_inputs(B, T, H, dk, dv, seed_ids=(72,), gate="slow")
