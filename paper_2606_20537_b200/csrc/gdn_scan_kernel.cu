@@ -239,9 +239,13 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
         tma_prefetch_desc(&tq); tma_prefetch_desc(&tk); tma_prefetch_desc(&tv);
     }
     if (warp == 2) tmem_alloc(tmem_slot, L::tmem_cols);
-    // the T staging buffer: the blocks above the diagonal are never written, so they are zeroed once
+    // Without a cluster (csz = 1: calls of up to kGdnShortT tokens, ONE chunk) there is nobody to push to: the T warps write the
+    // inverse straight into operand slot 0 and arrive on its barrier themselves (no staging, no push, no slot flow control).
+    const bool direct = csz == 1;
+    if (direct && n_chunks > 1) __trap();   // the host launches without a cluster for one-chunk calls only
+    // the T staging buffer (the slot in direct mode): the blocks above the diagonal are never written, so they are zeroed once
     for (uint32_t i = threadIdx.x; i < L::t_bytes / 16; i += L::kThreads)
-        reinterpret_cast<uint4*>(sm + L::tstage_off)[i] = make_uint4(0, 0, 0, 0);
+        reinterpret_cast<uint4*>(sm + (direct ? L::t_off : L::tstage_off))[i] = make_uint4(0, 0, 0, 0);
     fence_proxy_async_smem();
     tc_fence_before_sync();
     cluster_sync();   // every CTA's barriers are initialised before a peer copies a T into it or arrives on them
@@ -373,7 +377,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
         const uint64_t dW0 = smem_desc(sm_a + L::wv_off, 128, L::op_sbo, kSwzNone);
         for (uint32_t c = 0; c < n_chunks; ++c) {
             const uint32_t s = c % NS, sb = c & 1;
-            if (lane == 0) mbar_arrive_expect_tx(&bars[BI.t_full + sb], L::t_bytes);   // T(c): pushed by CTA c % csz (bulk copy into slot sb)
+            if (lane == 0 && !direct) mbar_arrive_expect_tx(&bars[BI.t_full + sb], L::t_bytes);   // T(c): pushed by CTA c % csz (bulk copy into slot sb)
             GW_(0, mbar_wait(&bars[BI.full + s], (c / NS) & 1));
             if (c >= 1) GW_(1, mbar_wait(&bars[BI.x_read], (c - 1) & 1));
             GW_(2, mbar_wait(&bars[BI.s_full + sb], (c >> 1) & 1));
@@ -449,7 +453,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
         // owns only (all of the same parity when csz is even; without a cluster, csz = 1, every chunk), one phase per owned chunk c >= 2.  (On a warp of its own: the T warps
         // are typically a few chunks ahead of the chain, and waiting for the slot would hold up their next chunk.)
         uint32_t k_own = 0;
-        for (uint32_t c = rank; c < n_chunks; c += csz, ++k_own) {
+        for (uint32_t c = rank; c < n_chunks && !direct; c += csz, ++k_own) {
             GW_(0, mbar_wait_relaxed(&bars[BI.t_staged], k_own & 1));
             // phase of t_free[c % 2] here: the owned chunks before this one that used the slot and had a predecessor (c' >= 2)
             if (c >= 2) GW_(1, mbar_wait_relaxed(&bars[BI.t_free + (c & 1)], (csz > 1 ? k_own - (rank < 2 ? 1u : 0u) : (c - 2) >> 1) & 1));
@@ -487,7 +491,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
         auto blk = [](int r, int cc) { return (uint32_t)((16 * r) * L::a_pitch + (16 * cc) * 2); };
         uint8_t* ast = sm + L::a_off;
         const uint32_t a_hi = sm_a + L::a_off, a_lo = a_hi + L::a_term_bytes;
-        uint8_t* tbase = sm + L::tstage_off;
+        uint8_t* tbase = sm + (direct ? L::t_off : L::tstage_off);
         constexpr uint32_t idG = idesc_bf16(kGC, kGC, 0, 0);
         const uint64_t dKg = smem_desc(sm_a + L::a_off, 16, 1024, kSwz128);
         uint32_t k_own = 0;                                // owned chunks done: the phase of this pipeline's own barriers
@@ -715,7 +719,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             GSEG(5);
             if (I == 0 && lane == 0) {
                 if (c + csz < n_chunks) load_k(c + csz);
-                mbar_arrive(&bars[BI.t_staged]);   // the push warp takes it from here: these warps go on with the next owned chunk
+                mbar_arrive(&bars[direct ? BI.t_full : BI.t_staged]);   // the push warp takes it from here: these warps go on with the next owned chunk
             }
             __syncwarp();
             GSEG(2);
