@@ -530,6 +530,16 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
         for (uint32_t c = rank; c < n_chunks; c += csz, ++k_own) {
             GSEG_START
             if (I == 0 && c + csz < n_chunks) load_raw(c + csz, k_own + 1);
+            if (I == 0) {   // G = K K^T, issued first: the MMAs run while the gate values are formed
+                mbar_wait_relaxed(&bars[BI.kg_full], k_own & 1);
+                tc_fence_after_sync();
+#pragma unroll 1
+                for (int ks = 0; ks < DK / 16; ++ks) {
+                    const uint32_t adv = (ks / 4) * L::half_bytes + (ks % 4) * 32;
+                    mma_bf16_ss_w(tb + L::tm_g, smem_desc_advance(dKg, adv), smem_desc_advance(dKg, adv), idG, ks > 0);
+                }
+                mma_commit_w(&bars[BI.g_done]);
+            }
             // gate values of the chunk from the raw a / beta that warp 8 copied in one owned chunk ahead (cp.async): lane l owns
             // tokens 2 l, 2 l + 1, then a warp scan.  (Each of the four warps keeps its own copy: no barrier.  The summation order
             // differs from the gate warp's, so these b agree with the chain's to an ulp of the exponent, not bit for bit; both are
@@ -552,16 +562,6 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             }
             const float bia = b2[ia], bib = b2[ib], bea = be[ia], beb = be[ib];
             GSEG(0);
-            if (I == 0) {   // G = K K^T
-                mbar_wait_relaxed(&bars[BI.kg_full], k_own & 1);
-                tc_fence_after_sync();
-#pragma unroll 1
-                for (int ks = 0; ks < DK / 16; ++ks) {
-                    const uint32_t adv = (ks / 4) * L::half_bytes + (ks % 4) * 32;
-                    mma_bf16_ss_w(tb + L::tm_g, smem_desc_advance(dKg, adv), smem_desc_advance(dKg, adv), idG, ks > 0);
-                }
-                mma_commit_w(&bars[BI.g_done]);
-            }
             mbar_wait_relaxed(&bars[BI.g_done], k_own & 1);   // (the MMAs have also finished reading the K tile: the staging matrix is free)
             tc_fence_after_sync();
             GSEG(1);
