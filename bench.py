@@ -757,7 +757,19 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
     cy = torch.empty((1, Tg, Cc), dtype=torch.float32, device=dev)
     conv_ms, _ = med_ms(lambda: esc.causal_conv(ctx, cx, cw, cst, cst, cy, 1, Tg, Tg, Cc, Wc, esc.CONV_SILU, stream=stream), n=7)
     conv_alg = Tg * Cc * 6
+    # the suffix after a restore with delta-rule layers: 18 chained 64-token calls (one per layer, own inputs and state; the calls
+    # chain by programmatic dependent launch), the shape of the step's suffix scan
+    gsuf = workload.SuffixInputs(N_LINEAR, SUFFIX, seed=12, device=dev)
+    gsbeta = torch.from_numpy(synth.gdn_beta(workload.B, SUFFIX, workload.H, seed_ids=(12,))).to(dev)
+    gsstate = [torch.zeros((workload.B, workload.H, 128, 128), dtype=torch.float32, device=dev) for _ in range(N_LINEAR)]
+
+    def gdn_suffix():
+        for n in range(N_LINEAR):
+            sq, sk, sv, sg = gsuf.dev[n]
+            esc.gdn_scan(ctx, key, sq, sk, sv, sg, gsbeta, gsstate[n], gsstate[n], gsuf.out[n], SUFFIX, SUFFIX, stream=stream)
+    gdn_suffix_ms, _ = med_ms(gdn_suffix, n=9, warm=2)
     res["gated_delta_rule"] = {"tokens": Tg, "ms": gdn_ms, "tokens_per_s": Tg / (gdn_ms * 1e-3),
+                               "suffix_18_layers_us": gdn_suffix_ms * 1e3, "suffix_us_per_layer": gdn_suffix_ms * 1e3 / N_LINEAR,
                                "roofline": {"kernel": "esc_gdn_scan_kernel<128> (chunked WY form, 64-token chunks, tcgen05 / TMEM / TMA, B1 H16 d128)", "bound": "hbm",
                                             "achieved": gdn_alg / (gdn_ms * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
                                             "frac": gdn_alg / (gdn_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "alg_bytes_per_launch": gdn_alg,
@@ -766,7 +778,7 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
                                "causal_conv": {"channels": Cc, "window": Wc, "us": conv_ms * 1e3, "GBps": conv_alg / (conv_ms * 1e-3) / 1e9,
                                                "frac_of_measured_peak": conv_alg / (conv_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
                                                "alg_bytes": "2 B read + 4 B written per element"}}
-    del gin, cx, cy
+    del gin, cx, cy, gsuf, gsstate
     # ---- BASELINE config 3: the 8k capsule (210 MiB) forked into 8 live sets (one launch: read once, write 8 times), then all
     # 8 rolled back to it (8 launches) ----
     P3, n3 = 8192, 8
