@@ -531,7 +531,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             GSEG_START
             if (I == 0 && c + csz < n_chunks) load_raw(c + csz, k_own + 1);
             if (I == 0) {   // G = K K^T, issued first: the MMAs run while the gate values are formed
-                mbar_wait_relaxed(&bars[BI.kg_full], k_own & 1);
+                mbar_wait(&bars[BI.kg_full], k_own & 1);
                 tc_fence_after_sync();
 #pragma unroll 1
                 for (int ks = 0; ks < DK / 16; ++ks) {
@@ -562,7 +562,7 @@ esc_gdn_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constan
             }
             const float bia = b2[ia], bib = b2[ib], bea = be[ia], beb = be[ib];
             GSEG(0);
-            mbar_wait_relaxed(&bars[BI.g_done], k_own & 1);   // (the MMAs have also finished reading the K tile: the staging matrix is free)
+            mbar_wait(&bars[BI.g_done], k_own & 1);   // (the MMAs have also finished reading the K tile: the staging matrix is free)
             tc_fence_after_sync();
             GSEG(1);
             uint32_t cur[8], nxt[8];
