@@ -768,8 +768,22 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
             sq, sk, sv, sg = gsuf.dev[n]
             esc.gdn_scan(ctx, key, sq, sk, sv, sg, gsbeta, gsstate[n], gsstate[n], gsuf.out[n], SUFFIX, SUFFIX, stream=stream)
     gdn_suffix_ms, _ = med_ms(gdn_suffix, n=9, warm=2)
+    # ... and the same as ONE captured plan with its restore node (esc_scan_args.kind = ESC_SCAN_GDN): warm rebuild at the 2k prefix
+    # for a model whose 18 linear layers are delta-rule layers (restore of the 66 MiB capsule + 18 x 64-token delta-rule scans)
+    sess.set.set_position(P_STEP)
+    gslab = sess.new_slab(P_STEP)
+    gcap = esc.snapshot(sess.set, P_STEP, CHUNK, gslab, stream=stream)
+    glayers = [esc.scan_args(key, *gsuf.dev[n], sess.states[n], sess.states[n], gsuf.out[n], SUFFIX, SUFFIX, CHUNK, beta=gsbeta)
+               for n in range(N_LINEAR)]
+    ggraph = esc.graph_capture(ctx, sess.set, P_STEP, glayers, stream)
+    ggraph.set_capsule(gcap, stream)
+    gdn_warm_ms, _ = med_ms(lambda: ggraph.launch(stream), n=15)
+    ggraph.destroy()
+    gcap.destroy()
+    del gslab
     res["gated_delta_rule"] = {"tokens": Tg, "ms": gdn_ms, "tokens_per_s": Tg / (gdn_ms * 1e-3),
                                "suffix_18_layers_us": gdn_suffix_ms * 1e3, "suffix_us_per_layer": gdn_suffix_ms * 1e3 / N_LINEAR,
+                               "warm_graph_2k_us": gdn_warm_ms * 1e3,
                                "roofline": {"kernel": "esc_gdn_scan_kernel<128> (chunked WY form, 64-token chunks, tcgen05 / TMEM / TMA, B1 H16 d128)", "bound": "hbm",
                                             "achieved": gdn_alg / (gdn_ms * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
                                             "frac": gdn_alg / (gdn_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "alg_bytes_per_launch": gdn_alg,

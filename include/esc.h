@@ -46,7 +46,7 @@
 extern "C" {
 #endif
 
-#define ESC_ABI_VERSION 2u
+#define ESC_ABI_VERSION 3u   /* 3: esc_scan_args gained `kind` (was reserved) and `beta`: gated delta-rule layers in a captured plan */
 
 /* ---- error codes -------------------------------------------------------------------- */
 #define ESC_OK               0
@@ -325,12 +325,18 @@ typedef struct esc_scan_args {
     esc_shape_key key;
     const void*  q; const void* k; const void* v; const float* g;
     const float* state_in; float* state_out; void* o;
-    uint64_t T; uint64_t t_stride; uint32_t chunk; uint32_t reserved;
+    uint64_t T; uint64_t t_stride; uint32_t chunk;
+    uint32_t kind;        /* ESC_SCAN_LINATTN (0): esc_linattn_scan;  ESC_SCAN_GDN (1): esc_gdn_scan (out_dtype F32) */
+    const float* beta;    /* ESC_SCAN_GDN: [B, T_stride, H] fp32 as in esc_gdn_scan; must be NULL for ESC_SCAN_LINATTN */
 } esc_scan_args;
+#define ESC_SCAN_LINATTN 0u
+#define ESC_SCAN_GDN 1u
 
 /*
  * Capture ONE CUDA graph = [restore node: capsule -> `live`] -> [scan node per layer, in
- * order].  `live` may be NULL (no restore node: a cold plan).  The restore node reads its
+ * order].  A layer is a linear-attention scan or a gated delta-rule scan (`kind`; a plan may mix
+ * them); the scan nodes chain by programmatic dependent launch.  `live` may be NULL (no restore
+ * node: a cold plan).  The restore node reads its
  * copy table from a device-resident descriptor, so the capsule can be swapped between replays
  * WITHOUT recapturing (the paper's "host overwrites a bound sub-buffer between replays" idiom,
  * PAPER.md:110).  That descriptor lives in `scratch_dev`: caller-owned device memory of at least

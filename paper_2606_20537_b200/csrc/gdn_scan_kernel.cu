@@ -1031,6 +1031,7 @@ static int launch_gdn_t(esc_ctx* ctx, const ScanShape& s, const void* q, const v
     using L = GdnCfg<DK>;
     const int rc0 = ensure_dyn_smem(ctx, kSlotGdn + (DK == 128 ? 0 : 1), esc_gdn_scan_kernel<DK>, (int)L::total);
     if (rc0 != ESC_OK) return rc0;
+    if (!state_out) return ESC_OK;   // prepare-only call (before a stream capture)
     CUtensorMap tq, tk, tv;
     const void* qq = T ? q : (const void*)state_out;   // T == 0: the maps are never dereferenced, any valid address will do
     const void* kk = T ? k : (const void*)state_out;

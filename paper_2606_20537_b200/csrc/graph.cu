@@ -70,14 +70,19 @@ int esc_graph_capture(esc_ctx* ctx, esc_bufset* live, uint64_t max_boundary, con
     std::vector<ScanShape> shapes(n_layers);
     for (uint32_t i = 0; i < n_layers; ++i) {
         const esc_scan_args& a = layers[i];
-        if (!decode_key(a.key, &shapes[i]) || !a.state_out || a.reserved != 0) return ESC_ERR_INVALID;
+        if (!decode_key(a.key, &shapes[i]) || !a.state_out || a.kind > ESC_SCAN_GDN) return ESC_ERR_INVALID;
+        const bool gdn = a.kind == ESC_SCAN_GDN;
+        if (gdn ? (a.T > 0 && !a.beta) : a.beta != nullptr) return ESC_ERR_INVALID;
+        if (gdn && shapes[i].out_dtype != ESC_DTYPE_F32) return ESC_ERR_UNSUPPORTED;
         if (a.T > 0 && (!a.q || !a.k || !a.v || !a.g || !a.o)) return ESC_ERR_INVALID;
         if (a.chunk != shapes[i].chunk) return ESC_ERR_MISMATCH;
         if (a.t_stride < a.T) return ESC_ERR_INVALID;
         const uintptr_t all = (uintptr_t)a.q | (uintptr_t)a.k | (uintptr_t)a.v | (uintptr_t)a.state_in |
                               (uintptr_t)a.state_out | (uintptr_t)a.o;
-        if ((all & 15u) || ((uintptr_t)a.g & 3u)) return ESC_ERR_UNALIGNED;
-        int rc = launch_scan(ctx, shapes[i], nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, nullptr);
+        if ((all & 15u) || (((uintptr_t)a.g | (uintptr_t)a.beta) & 3u)) return ESC_ERR_UNALIGNED;
+        // prepare-only calls (state_out == NULL): kernel attributes may not be set during a capture
+        int rc = gdn ? launch_gdn_mma(ctx, shapes[i], nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, nullptr)
+                     : launch_scan(ctx, shapes[i], nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, nullptr);
         if (rc != ESC_OK) return rc;
     }
 
@@ -112,7 +117,8 @@ int esc_graph_capture(esc_ctx* ctx, esc_bufset* live, uint64_t max_boundary, con
     if (live) rc = launch_copy_indirect(ctx, g->table_dev, grid, st);
     for (uint32_t i = 0; i < n_layers && rc == ESC_OK; ++i) {
         const esc_scan_args& a = layers[i];
-        rc = launch_scan(ctx, shapes[i], a.q, a.k, a.v, a.g, a.state_in, a.state_out, a.o, a.T, a.t_stride, st);
+        rc = a.kind == ESC_SCAN_GDN ? launch_gdn_mma(ctx, shapes[i], a.q, a.k, a.v, a.g, a.beta, a.state_in, a.state_out, (float*)a.o, a.T, a.t_stride, st)
+                                    : launch_scan(ctx, shapes[i], a.q, a.k, a.v, a.g, a.state_in, a.state_out, a.o, a.T, a.t_stride, st);
     }
     e = cudaStreamEndCapture(st, &g->graph);
     if (rc != ESC_OK || e != cudaSuccess) {

@@ -29,6 +29,7 @@ FORMAT_FP8_E4M3 = 1
 ALL_ROWS = 2**32 - 1
 RESTORE_DEQUANT_EAGER = 1
 CONV_SILU = 1
+SCAN_LINATTN, SCAN_GDN = 0, 1
 
 
 class EscError(RuntimeError):
@@ -55,7 +56,7 @@ class CapsuleInfo(C.Structure):
 class ScanArgs(C.Structure):
     _fields_ = [("key", C.c_uint64), ("q", C.c_void_p), ("k", C.c_void_p), ("v", C.c_void_p), ("g", C.c_void_p),
                 ("state_in", C.c_void_p), ("state_out", C.c_void_p), ("o", C.c_void_p),
-                ("T", C.c_uint64), ("t_stride", C.c_uint64), ("chunk", C.c_uint32), ("reserved", C.c_uint32)]
+                ("T", C.c_uint64), ("t_stride", C.c_uint64), ("chunk", C.c_uint32), ("kind", C.c_uint32), ("beta", C.c_void_p)]
 
 
 _P = C.c_void_p
@@ -360,10 +361,11 @@ def causal_conv(ctx, x, w, state_in, state_out, y, B, T, t_stride, Cch, W, flags
                                flags, _stream(stream)), "esc_causal_conv")
 
 
-def scan_args(key, q, k, v, g, state_in, state_out, o, T, t_stride, chunk):
+def scan_args(key, q, k, v, g, state_in, state_out, o, T, t_stride, chunk, beta=None):
+    """One layer of a captured plan: a linear-attention scan, or (beta given) a gated delta-rule scan."""
     a = ScanArgs(key, _ptr(q), _ptr(k), _ptr(v), _ptr(g), _ptr(state_in), _ptr(state_out), _ptr(o),
-                 T, t_stride, chunk, 0)
-    a._keep = (q, k, v, g, state_in, state_out, o)   # the struct holds raw addresses: keep the tensors alive with it
+                 T, t_stride, chunk, SCAN_LINATTN if beta is None else SCAN_GDN, _ptr(beta))
+    a._keep = (q, k, v, g, state_in, state_out, o, beta)   # the struct holds raw addresses: keep the tensors alive with it
     return a
 
 

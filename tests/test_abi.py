@@ -32,7 +32,7 @@ def test_header_symbols_all_exported(esc):
 
 
 def test_abi_version_and_strerror(esc):
-    assert esc.abi_version() == 2        # 2: esc_graph_capture takes caller-owned scratch, esc_plan_table_contains
+    assert esc.abi_version() == 3        # 3: esc_scan_args.kind / .beta (delta-rule layers in a captured plan)
     for code in range(0, -7, -1):
         s = esc.strerror(code)
         assert s and "?" not in s

@@ -6,7 +6,7 @@ import torch
 
 import oracle
 from paper_2606_20537_b200 import synth
-from gpu_util import (DEV, TOL_O, TOL_S, LiveSet, assert_state_close, bits_equal, err_o, err_s, esc_mod, sample_heads,
+from gpu_util import (to_dev, DEV, TOL_O, TOL_S, LiveSet, assert_state_close, bits_equal, err_o, err_s, esc_mod, sample_heads,
                       scan_dev_inputs)
 
 pytestmark = pytest.mark.gpu
@@ -96,6 +96,82 @@ def test_restore_plus_suffix_scan_graph(esc, ctx):
     assert err_o(outs[3].cpu().numpy(), o_ref) <= TOL_O
     assert_state_close(states[3], s_ref)
     graph.destroy()
+
+
+def test_delta_rule_layers_in_a_captured_plan(esc, ctx):
+    """esc_scan_args.kind = ESC_SCAN_GDN: the restore node followed by one gated delta-rule scan per layer (the recurrence of the
+    paper's own model family) replayed as ONE graph; bit-identical to restore + esc_gdn_scan calls, capsule
+    swapped without recapture, a mixed plan (delta-rule and linear-attention layers) accepted, one layer against the oracle."""
+    P = 2048
+    live, lin = _hybrid_live(esc, ctx, P + SUFFIX, 5)
+    states = [live.dev[i].view(torch.float32).view(B, H, DK, DV) for i in lin]
+    key = esc.shape_key_make(B, H, DK, DV, esc.DTYPE_BF16, esc.DTYPE_F32, CHUNK)
+    ins = [synth.scan_inputs(B, SUFFIX, H, DK, DV, seed_ids=(61, n), gate="slow") for n in range(len(lin))]
+    betas = [synth.gdn_beta(B, SUFFIX, H, seed_ids=(61, n)) for n in range(len(lin))]
+    dev_ins = [scan_dev_inputs(si) for si in ins]
+    dev_betas = [to_dev(b_) for b_ in betas]
+    outs = [torch.zeros((B, SUFFIX, H, DV), dtype=torch.float32, device=DEV) for _ in lin]
+    for n, i in enumerate(lin):
+        live.set_row(i, synth.scan_state(B, H, DK, DV, seed_ids=(62, n), scale=0.3))
+    slab_a = torch.empty(live.set.capsule_bytes(P)[0], dtype=torch.uint8, device=DEV)
+    cap_a = esc.snapshot(live.set, P, CHUNK, slab_a)
+    s0_a = [s.clone() for s in states]
+    for n, i in enumerate(lin):
+        live.set_row(i, synth.scan_state(B, H, DK, DV, seed_ids=(63, n), scale=0.3))
+    slab_b = torch.empty_like(slab_a)
+    cap_b = esc.snapshot(live.set, P, CHUNK, slab_b)
+    torch.cuda.synchronize()
+    gdn_layer = lambda n: n % 3 != 2   # a mixed plan: every third layer is a linear-attention layer
+
+    def by_verbs(cap):
+        esc.restore(live.set, cap)
+        for n in range(len(lin)):
+            q, k, v, g = dev_ins[n]
+            if gdn_layer(n):
+                esc.gdn_scan(ctx, key, q, k, v, g, dev_betas[n], states[n], states[n], outs[n], SUFFIX, SUFFIX)
+            else:
+                esc.linattn_scan(ctx, key, q, k, v, g, states[n], states[n], outs[n], SUFFIX, SUFFIX, CHUNK)
+        torch.cuda.synchronize()
+        return [o.clone() for o in outs], [s.clone() for s in states]
+
+    exp_a, exp_b = by_verbs(cap_a), by_verbs(cap_b)
+    assert not bits_equal(exp_a[0][0], exp_b[0][0])
+    stream = torch.cuda.Stream()
+    layers = [esc.scan_args(key, *dev_ins[n], states[n], states[n], outs[n], SUFFIX, SUFFIX, CHUNK,
+                            beta=dev_betas[n] if gdn_layer(n) else None) for n in range(len(lin))]
+    graph = esc.graph_capture(ctx, live.set, P, layers, stream)
+    for cap, (exp_o, exp_s) in ((cap_a, exp_a), (cap_b, exp_b), (cap_a, exp_a)):
+        for o in outs:
+            o.fill_(float("nan"))
+        for s_ in states:
+            s_.fill_(float("nan"))
+        torch.cuda.synchronize()
+        graph.set_capsule(cap, stream)
+        graph.launch(stream)
+        stream.synchronize()
+        for n in range(len(lin)):
+            assert bits_equal(outs[n], exp_o[n]) and bits_equal(states[n], exp_s[n]), n
+    q, k, v, g = ins[0].as_f32()
+    o_ref, s_ref = oracle.gdn_recurrence(q, k, v, g, betas[0], s0_a[0].cpu().numpy().astype(np.float64))
+    assert err_o(outs[0].cpu().numpy(), o_ref) <= TOL_O
+    assert_state_close(states[0], s_ref)
+    graph.destroy()
+    # argument contract: beta on a linear-attention layer, a delta-rule layer without beta, an unknown kind
+    bad = esc.scan_args(key, *dev_ins[0], states[0], states[0], outs[0], SUFFIX, SUFFIX, CHUNK)
+    bad.beta = dev_betas[0].data_ptr()
+    with pytest.raises(esc.EscError):
+        esc.graph_capture(ctx, None, 0, [bad], stream)
+    bad = esc.scan_args(key, *dev_ins[0], states[0], states[0], outs[0], SUFFIX, SUFFIX, CHUNK, beta=dev_betas[0])
+    bad.beta = None
+    with pytest.raises(esc.EscError):
+        esc.graph_capture(ctx, None, 0, [bad], stream)
+    bad = esc.scan_args(key, *dev_ins[0], states[0], states[0], outs[0], SUFFIX, SUFFIX, CHUNK)
+    bad.kind = 7
+    with pytest.raises(esc.EscError):
+        esc.graph_capture(ctx, None, 0, [bad], stream)
+    cap_a.destroy()
+    cap_b.destroy()
+    live.set.destroy()
 
 
 def test_cold_plan_graph_matches_direct_calls(esc, ctx):
