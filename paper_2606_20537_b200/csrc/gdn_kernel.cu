@@ -3,6 +3,7 @@
 // hybrid-model family ("recurrent state and convolution state are a fold over the entire prefix [4, 13]";
 // DESIGN.md reading 25).  The delta-rule kernel itself is gdn_mma_kernel.cu.
 #include <cuda_bf16.h>
+#include <string.h>
 
 #include "esc_internal.h"
 #include "sm100_ptx.cuh"
@@ -25,7 +26,7 @@ __device__ __forceinline__ float rcp_approx(float x) {
 // SiLU is s / (1 + e^-s) with ex2.approx and the approximate divide (2 ulp each; the full-precision expf + IEEE divide
 // made the kernel ALU-bound: 150 -> 120 us on their own); for s < -88 the quotient is -0 where the exact value is ~ -1e-37.
 constexpr int kConvMaxW = 8;
-constexpr int kConvRun = 64;      // tokens per thread
+constexpr int kConvRun = 64;      // tokens per thread (long calls; short calls take shorter runs, see conv_run_tokens)
 constexpr int kConvThreads = 128;
 constexpr int kConvCPT = 4;       // channels per thread (8-byte bf16 vectors: a warp reads 256 contiguous bytes of a token row)
 constexpr int kConvU = 4;         // vectors per batch (one batch in flight per thread while the previous one is computed)
@@ -43,13 +44,18 @@ __device__ __forceinline__ uint2 ld_stream8(const __nv_bfloat16* p) {
 template <int W>
 __global__ void __launch_bounds__(kConvThreads) esc_causal_conv_kernel(const __nv_bfloat16* __restrict__ x, const float* __restrict__ w,
                                                                        const float* __restrict__ state_in, float* __restrict__ y,
-                                                                       uint64_t T, uint64_t t_stride, uint32_t C, uint32_t silu) {
+                                                                       uint64_t T, uint64_t t_stride, uint32_t C, uint32_t silu, uint32_t run,
+                                                                       float* state_out) {
     constexpr int P = kConvCPT, U = kConvU;
+    // programmatic dependent launch: the next kernel of the stream may be placed while this one runs; this kernel touches global
+    // memory only after its predecessor has completed
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const uint32_t cg = blockIdx.x * kConvThreads + threadIdx.x;   // channel group
     if (cg >= C / P) return;
     const uint32_t b = blockIdx.z;
-    const uint64_t t_begin = (uint64_t)blockIdx.y * kConvRun;
-    const uint32_t n_tok = (uint32_t)(t_begin + kConvRun < T ? kConvRun : T - t_begin);
+    const uint64_t t_begin = (uint64_t)blockIdx.y * run;
+    const uint32_t n_tok = (uint32_t)(t_begin + run < T ? run : T - t_begin);
     const __nv_bfloat16* xp = x + ((size_t)b * t_stride + t_begin) * C + cg * P;
     float* yp = y + ((size_t)b * T + t_begin) * C + cg * P;
     uint2 nxt[U];   // the batch in flight
@@ -110,9 +116,39 @@ __global__ void __launch_bounds__(kConvThreads) esc_causal_conv_kernel(const __n
         xp += (size_t)U * C;
         yp += (size_t)U * C;
     }
+    // The carried window after the call (the last W-1 inputs, T >= W-1: the host passes state_out only then), written by the threads
+    // of the FIRST run: they are the only ones that read state_in (a run is at least W-1 tokens long), and they have read it by
+    // now, so state_out may alias state_in.  (One launch instead of two for the 64-token suffix call.)
+    // (Loading these W-1 vectors up front, with the thread's other loads, saves a memory round trip on a 64-token call — 5.3 -> 5.1 us
+    // chained — but costs 8 registers and a CTA of occupancy on long calls.)
+    if (state_out != nullptr && blockIdx.y == 0) {
+#pragma unroll
+        for (int i = 0; i < W - 1; ++i) {
+            float v4[P];
+            bf16x4_to_f32(ld_stream8(x + ((size_t)b * t_stride + (T - (uint64_t)(W - 1) + i)) * C + cg * P), v4);
+#pragma unroll
+            for (int j = 0; j < P; ++j) state_out[((size_t)b * C + cg * P + j) * (W - 1) + i] = v4[j];
+        }
+    }
 }
 
-typedef void (*ConvKernelFn)(const __nv_bfloat16*, const float*, const float*, float*, uint64_t, uint64_t, uint32_t, uint32_t);
+typedef void (*ConvKernelFn)(const __nv_bfloat16*, const float*, const float*, float*, uint64_t, uint64_t, uint32_t, uint32_t, uint32_t, float*);
+
+// Tokens a thread walks.  64 for long calls (every input vector loaded once, + W-1 to prime the window).  A short call (the suffix
+// after a restore: 64 tokens) would then be 12 CTAs walking 64 tokens one after the other: 21 us, all of it latency.  Short calls
+// take runs of as few as 4 tokens (one batch in flight), so that the grid still has a few CTAs per SM: the extra priming loads hit L2.
+// The arithmetic of an output does not depend on the run it falls in: same bits.
+static uint32_t conv_run_tokens(uint32_t B, uint64_t T, uint32_t C, uint32_t W, uint32_t sm_count) {
+    const uint64_t col_blocks = (C / kConvCPT + kConvThreads - 1) / kConvThreads;
+    const uint64_t want = 4ull * (sm_count ? sm_count : 148u);                  // CTAs
+    uint64_t run = (T * col_blocks * B) / want;                                  // tokens per run that give `want` CTAs
+    run = run / kConvU * kConvU;
+    const uint64_t run_min = (W - 1 + kConvU - 1) / kConvU * kConvU;   // >= W-1: only the first run reaches back into the carried window
+    if (run < run_min) run = run_min;
+    if (run < (uint64_t)kConvU) run = kConvU;
+    if (run > (uint64_t)kConvRun) run = kConvRun;
+    return (uint32_t)run;
+}
 static ConvKernelFn conv_kernel_for(uint32_t W) {
     switch (W) {
         case 1: return esc_causal_conv_kernel<1>;
@@ -169,13 +205,24 @@ int esc_causal_conv(esc_ctx* ctx, const void* x, const float* w, const float* st
     if ((((uintptr_t)x | (uintptr_t)y) & 15u) || (((uintptr_t)w | (uintptr_t)state_in | (uintptr_t)state_out) & 3u)) return ESC_ERR_UNALIGNED;
     if (T > 0 && B > 65535) return ESC_ERR_UNSUPPORTED;
     ESC_ON_DEVICE(ctx);
+    const bool fused_state = W > 1 && T >= W - 1;   // the conv kernel's first run writes the carried window itself
     if (T > 0) {
-        dim3 grid((C / kConvCPT + kConvThreads - 1) / kConvThreads, (uint32_t)((T + kConvRun - 1) / kConvRun), B);
-        conv_kernel_for(W)<<<grid, kConvThreads, 0, (cudaStream_t)stream>>>((const __nv_bfloat16*)x, w, state_in, y, T, t_stride, C,
-                                                                            flags & ESC_CONV_SILU);
-        ESC_CUDA(cudaGetLastError());
+        const uint32_t run = conv_run_tokens(B, T, C, W, (uint32_t)ctx->sm_count);
+        dim3 grid((C / kConvCPT + kConvThreads - 1) / kConvThreads, (uint32_t)((T + run - 1) / run), B);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid;
+        cfg.blockDim = dim3(kConvThreads);
+        cfg.stream = (cudaStream_t)stream;
+        cudaLaunchAttribute attr[1];
+        memset(attr, 0, sizeof attr);
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol.* in the kernel
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        ESC_CUDA(cudaLaunchKernelEx(&cfg, conv_kernel_for(W), (const __nv_bfloat16*)x, w, state_in, y, T, t_stride, C,
+                                    (uint32_t)(flags & ESC_CONV_SILU), run, fused_state ? state_out : (float*)nullptr));
     }
-    if (W > 1 && (T > 0 || state_in != state_out)) {
+    if (W > 1 && !fused_state && (T > 0 || state_in != state_out)) {
         const uint64_t n = (uint64_t)B * C;
         esc_conv_state_kernel<<<(uint32_t)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>((const __nv_bfloat16*)x, state_in, state_out, B, T,
                                                                                            t_stride, C, W);
