@@ -757,6 +757,10 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
     cy = torch.empty((1, Tg, Cc), dtype=torch.float32, device=dev)
     conv_ms, _ = med_ms(lambda: esc.causal_conv(ctx, cx, cw, cst, cst, cy, 1, Tg, Tg, Cc, Wc, esc.CONV_SILU, stream=stream), n=7)
     conv_alg = Tg * Cc * 6
+    # the same convolution over a 64-token suffix (a delta-rule layer's suffix call): latency, not bandwidth
+    sx = torch.randn((1, SUFFIX, Cc), device=dev).to(torch.bfloat16)
+    sy = torch.empty((1, SUFFIX, Cc), dtype=torch.float32, device=dev)
+    conv_short_ms, _ = med_ms(lambda: esc.causal_conv(ctx, sx, cw, cst, cst, sy, 1, SUFFIX, SUFFIX, Cc, Wc, esc.CONV_SILU, stream=stream), n=9)
     # the suffix after a restore with delta-rule layers: 18 chained 64-token calls (one per layer, own inputs and state; the calls
     # chain by programmatic dependent launch), the shape of the step's suffix scan
     gsuf = workload.SuffixInputs(N_LINEAR, SUFFIX, seed=12, device=dev)
@@ -789,7 +793,7 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
                                             "frac": gdn_alg / (gdn_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "alg_bytes_per_launch": gdn_alg,
                                             "traffic": measured_traffic("esc_gdn_scan_kernel")[0], "traffic_note": measured_traffic("esc_gdn_scan_kernel")[1],
                                             "note": "bound by the per-chunk dependency chain S -> X -> R -> Wm -> W~ -> U -> S (three MMA groups and three register passes) and by the off-chain inverse of the 64 x 64 triangular system, one CTA per (b, h, 16 d_v columns); not HBM"},
-                               "causal_conv": {"channels": Cc, "window": Wc, "us": conv_ms * 1e3, "GBps": conv_alg / (conv_ms * 1e-3) / 1e9,
+                               "causal_conv": {"channels": Cc, "window": Wc, "us": conv_ms * 1e3, "us_64_token_call": conv_short_ms * 1e3, "GBps": conv_alg / (conv_ms * 1e-3) / 1e9,
                                                "frac_of_measured_peak": conv_alg / (conv_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
                                                "alg_bytes": "2 B read + 4 B written per element"}}
     del gin, cx, cy, gsuf, gsstate
