@@ -203,6 +203,13 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (threadIdx.x == 0) TC_TRACE(11, 0);
 
+    // the waits of the roles that run ahead of the pipeline (producer, gate warp).  Long calls poll tightly: a back-off of 64 ns
+    // in these waits costs them 1.5 % (r02: 0.329 -> 0.334 of roofline at B 1, 16k); the one-chunk launches of the suffix path
+    // are faster WITH it (67.6 vs 69.6 us per 18 layers): fewer polls beside the few warps that have work.
+    auto wait_ahead = [&](uint64_t* bar, uint32_t parity) {
+        if constexpr (CS > 1) mbar_wait(bar, parity);
+        else mbar_wait_relaxed(bar, parity);
+    };
     // commit that every CTA of the cluster must see (stage reuse: every CTA writes into every CTA's stage)
     auto commit_all = [&](uint64_t* bar) {   // warp-uniform (every lane calls it, one elected lane issues)
         if constexpr (CS > 1) mma_commit_mc_w(bar, kAll);
@@ -267,7 +274,7 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
                 const int t0 = (int)(c * kC);
                 uint8_t* st = sm + L::stage_off + s * L::stage_bytes;
                 // the stage is free once the [P|O1] and U issuers of all CS CTAs have committed chunk c - NS
-                if (CS > 1 || c >= (uint32_t)NS) PW(0, mbar_wait_relaxed(&bars[BI.empty + s], ((c / NS) & 1) ^ 1));   // (a short call's first round: fresh)
+                if (CS > 1 || c >= (uint32_t)NS) PW(0, wait_ahead(&bars[BI.empty + s], ((c / NS) & 1) ^ 1));   // (a short call's first round: fresh)
                 uint64_t* full = &bars[BI.full + s];
                 mbar_arrive_expect_tx(full, L::q_bytes + L::k_tile_bytes);   // arrives in CS row slices, one from each CTA
                 if constexpr (CS > 1) {
@@ -288,8 +295,8 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
                 // V tiles have a ring of their own: O2 (the end of the score path) reads V from it, so a Q/K stage is
                 // released as soon as [P|O1] and U are done with it
                 if (CS > 1 || c >= (uint32_t)NV) {
-                    PW(1, mbar_wait_relaxed(&bars[BI.v_read + vi], ((c / NV) & 1) ^ 1));      // the V~ warps and O2 of chunk c - NV
-                    PW(1, mbar_wait_relaxed(&bars[BI.o2_done + vi], ((c / NV) & 1) ^ 1));     // are done with V tile vi
+                    PW(1, wait_ahead(&bars[BI.v_read + vi], ((c / NV) & 1) ^ 1));      // the V~ warps and O2 of chunk c - NV
+                    PW(1, wait_ahead(&bars[BI.o2_done + vi], ((c / NV) & 1) ^ 1));     // are done with V tile vi
                 }
                 mbar_arrive_expect_tx(&bars[BI.v_full + vi], L::v_bytes);
                 tma_load_4d(sm + L::v_off + vi * L::v_bytes, &tv, &bars[BI.v_full + vi], (int)dv0, (int)h, t0, (int)b);
@@ -329,7 +336,7 @@ esc_scan_kernel(const __grid_constant__ CUtensorMap tq, const __grid_constant__ 
             const float prev = __shfl_up_sync(0xffffffffu, incl, 1);
             const float excl = (lane % GL) ? prev : 0.f;
             const uint32_t slot = bt & 1;
-            if (CS > 1 || bt >= 2) PW(0, mbar_wait_relaxed(&bars[BI.g_empty + slot], ((bt >> 1) & 1) ^ 1));
+            if (CS > 1 || bt >= 2) PW(0, wait_ahead(&bars[BI.g_empty + slot], ((bt >> 1) & 1) ^ 1));
             float* b2 = gate + slot * 2 * kGateBatch;
             float* eb = b2 + kGateBatch;
 #pragma unroll
