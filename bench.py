@@ -332,6 +332,7 @@ def run_esc(args):
     layers, key = workload.scan_layers(sess, inputs, CHUNK)
     graph = esc.graph_capture(ctx, sess.set, P_STEP, layers, stream)
     slabs = [sess.new_slab(P_STEP) for _ in range(N_CAPSULES)]
+    torch.cuda.synchronize()
     caps = [esc.snapshot(sess.set, P_STEP, CHUNK, s, stream=stream) for s in slabs]
     flush = torch.empty(FLUSH_BYTES, dtype=torch.uint8, device=dev)
     flush_sink = torch.zeros(1, dtype=torch.float32, device=dev)
@@ -624,6 +625,7 @@ def extras(args, torch, esc, workload, ctx, stream, flush_l2, pk, dev):
     warm_layers, key = workload.scan_layers(sess, suffix, CHUNK)
 
     def med_ms(fn, n=15, warm=2):
+        torch.cuda.synchronize()      # inputs made on the default stream are complete before `stream` reads them
         for _ in range(warm):
             fn()
         pairs = []

@@ -285,6 +285,7 @@ def test_config2_capsule_and_warm_graph_equal_cold_graph(esc, ctx):
     o_cold = [torch.full((B, T, H, DV), float("nan"), dtype=torch.float32, device=DEV) for _ in range(n_lin)]
     cold = esc.graph_capture(ctx, None, 0, [esc.scan_args(key, *dev_ins[n], None, s_cold[n], o_cold[n], T, T, CHUNK)
                                             for n in range(n_lin)], stream)
+    torch.cuda.synchronize()      # the inputs and the NaN fills were enqueued on the default stream; `stream` does not wait for it
     cold.launch(stream)
     stream.synchronize()
     cold.destroy()
@@ -383,6 +384,7 @@ def test_plan_table_lru_and_padded_bucket(esc):
     assert e.value.code == esc.ERR_INVALID
     plan = ctx.plan_get(pk[0])                               # hit; pk[0] becomes most recently used
     assert plan is not None
+    torch.cuda.synchronize()                                 # default-stream set-up before the side stream's launch
     plan.launch(stream)
     stream.synchronize()
     assert bits_equal(o[:, :T], o_ref) and bits_equal(state, s_ref)
@@ -419,6 +421,7 @@ def test_graph_scratch_and_capacity_contract(esc, ctx):
     scratch = torch.full((need,), 0xAB, dtype=torch.uint8, device=DEV)    # garbage in the scratch must not matter
     graph = esc.graph_capture(ctx, live.set, 128, [], stream, scratch=scratch)
     slab = torch.empty(live.set.capsule_bytes(192)[0], dtype=torch.uint8, device=DEV)
+    torch.cuda.synchronize()
     cap_late = esc.snapshot(live.set, 192, 64, slab, stream=stream)
     with pytest.raises(esc.EscError) as e:
         graph.set_capsule(cap_late, stream)                  # boundary 192 > max_boundary 128
