@@ -20,16 +20,21 @@ __device__ __forceinline__ float rcp_approx(float x) {
 // Bound: HBM (2 B read + 4 B written per element).  A thread owns 4 consecutive channels (one 8-byte bf16 vector; a
 // warp reads 256 contiguous bytes of a token row) and walks kConvRun consecutive tokens with the W-1 previous input
 // vectors and its 4 x W taps in registers, so every input vector is loaded once per run (+ W-1 to prime the window).
-// The loads are software-pipelined: the kConvU vectors of the next batch are issued (L1 no-allocate) before the current
-// batch is computed and stored, so a thread always has a batch in flight (r01u: 150 -> 113 us at 16 448 x 6144, W = 4;
-// without the pipelining the loop is issue -> wait -> compute -> store and the SM's bytes in flight drop between batches).
+// The loads go through a per-thread ring in shared memory filled by cp.async (kConvRing batches of kConvU vectors; a thread
+// copies and reads only its OWN slots, so there is no barrier, only cp.async.wait_group): kConvRing - 1 batches are in flight
+// per thread without being held in registers.  History at 16 448 x 6144, W = 4: issue -> wait -> compute -> store 150 us; the
+// next batch loaded into registers before the current one is computed 113 us (r01u); packed fp32 and the fused window write
+// 106.5-108.5 us; the ring 104.4 us (three, four and six batches the same, eight slower: shared memory then limits the CTAs per
+// SM); runs of 48 tokens instead of 64 (four waves of shorter CTAs: the SMs idled 7 % of the launch at its ramp and tail)
+// 102.4 us = 5.92 TB/s.
 // SiLU is s / (1 + e^-s) with ex2.approx and the approximate divide (2 ulp each; the full-precision expf + IEEE divide
 // made the kernel ALU-bound: 150 -> 120 us on their own); for s < -88 the quotient is -0 where the exact value is ~ -1e-37.
 constexpr int kConvMaxW = 8;
-constexpr int kConvRun = 64;      // tokens per thread (long calls; short calls take shorter runs, see conv_run_tokens)
+constexpr int kConvRun = 48;      // tokens per thread (long calls; short calls take shorter runs, see conv_run_tokens)
 constexpr int kConvThreads = 128;
 constexpr int kConvCPT = 4;       // channels per thread (8-byte bf16 vectors: a warp reads 256 contiguous bytes of a token row)
 constexpr int kConvU = 4;         // vectors per batch (one batch in flight per thread while the previous one is computed)
+constexpr int kConvRing = 4;      // batches in a thread's shared-memory ring (kConvRing - 1 in flight)
 
 __device__ __forceinline__ void bf16x4_to_f32(const uint2& raw, float (&x)[4]) {
     x[0] = __uint_as_float(raw.x << 16); x[1] = __uint_as_float(raw.x & 0xFFFF0000u);
@@ -58,10 +63,19 @@ __global__ void __launch_bounds__(kConvThreads) esc_causal_conv_kernel(const __n
     const uint32_t n_tok = (uint32_t)(t_begin + run < T ? run : T - t_begin);
     const __nv_bfloat16* xp = x + ((size_t)b * t_stride + t_begin) * C + cg * P;
     float* yp = y + ((size_t)b * T + t_begin) * C + cg * P;
-    uint2 nxt[U];   // the batch in flight
+    // a ring of NBR batches per thread in shared memory, filled by cp.async: each thread copies and reads its OWN slots (no
+    // barrier, only cp.async.wait_group), NBR - 1 batches in flight without holding them in registers
+    constexpr int NBR = kConvRing;
+    __shared__ uint2 ring[NBR * U * kConvThreads];
+    uint2* my = ring + threadIdx.x;
+    auto issue = [&](uint32_t batch) {   // tokens [U batch, U batch + U) of the run into slot batch % NBR
 #pragma unroll
-    for (int u = 0; u < U; ++u)
-        if ((uint32_t)u < n_tok) nxt[u] = ld_stream8(xp + (size_t)u * C);
+        for (int u = 0; u < U; ++u)
+            if (batch * U + u < n_tok) ptx::cp_async_8(my + ((batch % NBR) * U + u) * kConvThreads, xp + (size_t)(batch * U + u) * C);
+        ptx::cp_async_commit();
+    };
+#pragma unroll
+    for (int bb = 0; bb < NBR - 1; ++bb) issue(bb);
     float wt[W][P];   // wt[i][j] = tap i of channel P cg + j
 #pragma unroll
     for (int j = 0; j < P; ++j)
@@ -82,11 +96,11 @@ __global__ void __launch_bounds__(kConvThreads) esc_causal_conv_kernel(const __n
     }
     for (uint32_t t = 0; t < n_tok; t += U) {
         uint2 raw[U];
+        const uint32_t bi = t / U;
+        issue(bi + NBR - 1);                  // into the slot batch bi - 1 was read from (its values are consumed)
+        ptx::cp_async_wait_group<NBR - 1>();  // batch bi has landed
 #pragma unroll
-        for (int u = 0; u < U; ++u) raw[u] = nxt[u];
-#pragma unroll
-        for (int u = 0; u < U; ++u)
-            if (t + U + u < n_tok) nxt[u] = ld_stream8(xp + (size_t)(U + u) * C);
+        for (int u = 0; u < U; ++u) raw[u] = my[((bi % NBR) * U + u) * kConvThreads];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             if (t + u < n_tok) {
@@ -113,7 +127,6 @@ __global__ void __launch_bounds__(kConvThreads) esc_causal_conv_kernel(const __n
                     for (int j = 0; j < P; ++j) win[i][j] = win[i + 1][j];
             }
         }
-        xp += (size_t)U * C;
         yp += (size_t)U * C;
     }
     // The carried window after the call (the last W-1 inputs, T >= W-1: the host passes state_out only then), written by the threads
