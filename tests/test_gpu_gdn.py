@@ -157,7 +157,10 @@ def test_gdn_errors(esc, ctx):
                                           # short calls take short runs (4 or 8 tokens per thread) and the first run writes the carried
                                           # window itself: every window size, T below / at / above W - 1, T not a multiple of a run
                                           (1, 7, 512, 8, True), (1, 8, 512, 8, False), (2, 9, 1024, 8, True), (1, 13, 2048, 5, False),
-                                          (1, 3, 512, 4, True), (1, 4, 512, 4, False), (1, 67, 6144, 2, True), (2, 130, 6144, 7, True)])
+                                          (1, 3, 512, 4, True), (1, 4, 512, 4, False), (1, 67, 6144, 2, True), (2, 130, 6144, 7, True),
+                                          # long calls: full 48-token runs (the per-thread cp.async ring wraps three times), a ragged
+                                          # last run; the split at T // 2 takes 24-token runs
+                                          (1, 2500, 6144, 4, True), (2, 1203, 6144, 3, False)])
 def test_causal_conv_vs_oracle_and_continuation(esc, ctx, B, T, C, W, silu):
     x_bits, w, st = synth.conv_inputs(B, T, C, W, seed_ids=(80, T, C))
     x = to_dev(x_bits.view(np.int16)).view(torch.bfloat16)
