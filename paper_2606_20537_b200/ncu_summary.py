@@ -1,7 +1,7 @@
 """Summarise an Nsight Compute capture of the library's kernels as text and record its DRAM traffic.
 
     python -m paper_2606_20537_b200.ncu_summary REPORT.ncu-rep --name esc_scan_kernel_cold \
-        --out profiles/r02_scan_ncu_full.txt --command "<the ncu command that made the report>" [--launch 0]
+        --out profiles/r02_scan_w16_ncu_full.txt --command "<the ncu command that made the report>" [--launch 0]
 
 reads the report with `ncu -i REPORT --page raw --csv` (works without a GPU), writes the selected counters of one
 captured launch to --out (with the command, so the file names what made it), and stores that launch's
