@@ -165,11 +165,16 @@ def test_causal_conv_vs_oracle_and_continuation(esc, ctx, B, T, C, W, silu):
     x_bits, w, st = synth.conv_inputs(B, T, C, W, seed_ids=(80, T, C))
     x = to_dev(x_bits.view(np.int16)).view(torch.bfloat16)
     wd, s_in = to_dev(w), to_dev(st)
-    y = torch.full((B, T, C), float("nan"), dtype=torch.float32, device=DEV)
+    # y sits between two canaries: a store outside [B, T, C] (a run or a ring slot past the ragged end) would show
+    guard = 4096
+    ybuf = torch.full((guard + B * T * C + guard,), -12345.0, dtype=torch.float32, device=DEV)
+    y = ybuf[guard:guard + B * T * C].view(B, T, C)
+    y.fill_(float("nan"))
     s_out = torch.full((B, C, max(W - 1, 1)), float("nan"), dtype=torch.float32, device=DEV)
     flags = esc.CONV_SILU if silu else 0
     esc.causal_conv(ctx, x, wd, s_in if W > 1 else None, s_out, y, B, T, T, C, W, flags)
     torch.cuda.synchronize()
+    assert bool((ybuf[:guard] == -12345.0).all()) and bool((ybuf[guard + B * T * C:] == -12345.0).all())
     y_ref, s_ref = oracle.causal_conv(synth.bf16_bits_to_f32(x_bits), w, st.astype(np.float64) if W > 1 else None, silu=silu)
     assert np.abs(y.cpu().numpy() - y_ref).max() <= 1e-5 * max(1.0, np.abs(y_ref).max())
     if W > 1:
