@@ -1,7 +1,7 @@
 // Short causal convolution with carried window, and the C entry points of the gated delta-rule row (include/esc.h:
 // esc_gdn_scan, esc_causal_conv) — SURVEY.md §8(f) #1: the recurrence and the convolution state of the paper's actual
 // hybrid-model family ("recurrent state and convolution state are a fold over the entire prefix [4, 13]";
-// DESIGN.md reading 25).  The delta-rule kernel itself is gdn_mma_kernel.cu.
+// DESIGN.md reading 25).  The delta-rule kernel itself is gdn_scan_kernel.cu.
 #include <cuda_bf16.h>
 #include <string.h>
 
